@@ -1,0 +1,173 @@
+/* md.h — C ABI of the B200-native EAM / TB-SMA molecular-dynamics hot path.
+ *
+ * Method: Hou et al., "Molecular dynamics simulations with many-body potentials on multiple
+ * GPUs - the implementation, package and performance", arxiv 1212.6332.  Citations below are
+ * PAPER.md:<line> of the extracted text plus the section / equation / figure.
+ *
+ *   E_i = F(sum_j rho(r_ij)) + 1/2 sum_j V(r_ij)                          eq.(1)
+ *   f_i = -sum_j [F'(rho_i)+F'(rho_j)] rho'(r_ij) r_ij/r_ij - sum_j V'(r_ij) r_ij/r_ij   eq.(3)
+ *
+ * evaluated on one GPU by: cell binning + re-ordering into cell order (sec. 3.2, PAPER.md:137-145,
+ * done there on the host, here on the device), a full Verlet neighbour list over the 27-cell
+ * stencil (Fig.3), a density pass (Fig.5), a
+ * force pass with virial (Fig.6) and a time integrator (sec. 3.3; here
+ * velocity-Verlet with a skin/2 displacement-triggered rebuild instead of the paper's fixed
+ * 10-step interval), optionally for many independent periodic boxes packed into
+ * one system (sec. 4.4).
+ *
+ * GENERAL CONVENTIONS
+ *  - Units: eV, Angstrom, fs, amu.  All floating point is IEEE double, all indices int32.
+ *  - Every function returns an int status: MD_OK (0) or a negative MD_E* code.  Nothing
+ *    throws or aborts across this boundary.  md_strerror() gives text.
+ *  - POINTERS.  Every array argument may be a DEVICE pointer (e.g. a torch CUDA tensor's
+ *    data_ptr()) or a HOST pointer (pageable or pinned); the library asks the CUDA runtime
+ *    which (cudaPointerGetAttributes) and stages host buffers through its workspace with
+ *    cudaMemcpyAsync on the system's stream.  Calls that take a host pointer synchronise the
+ *    stream before returning; calls with device pointers only enqueue work.  md_desc.mass and the
+ *    TB-SMA parameter arrays are always HOST (a few doubles).
+ *  - OWNERSHIP.  md_create copies every input; the caller keeps its buffers.  Outputs are
+ *    written into caller-provided buffers; any output pointer may be NULL (= skip).
+ *    The library never allocates device memory: the caller provides ONE workspace allocation
+ *    of md_workspace_bytes() bytes (256-byte aligned) that must outlive the system.
+ *  - ORDER.  Inputs and outputs are in CALLER atom order, AoS [n_atoms][3]; internally atoms
+ *    are kept in cell order (the paper's hGID map).  With n_boxes > 1, box b owns
+ *    atoms [b*n_atoms/n_boxes, (b+1)*n_atoms/n_boxes).
+ *  - STREAM.  All work is enqueued on md_desc.stream (a cudaStream_t; NULL = legacy default).
+ *  - ERRORS found on the device (neighbour overflow, non-finite coordinate, coincident atoms)
+ *    are sticky flags returned by the next call that synchronises: md_get_stats, any getter
+ *    into host memory, md_get_energies.
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns MD_ECUDA.
+ */
+#ifndef PAPER_1212_6332_B200_MD_H
+#define PAPER_1212_6332_B200_MD_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  MD_OK = 0,
+  MD_EINVAL = -1,      /* bad argument (NULL, size <= 0, type out of range, workspace too small ...) */
+  MD_EBOX = -2,        /* some L_a < 3 (cutoff+skin): the 27-cell stencil would alias */
+  MD_EOVERFLOW = -3,   /* an atom has more neighbours than the list capacity (the paper's MN) */
+  MD_ENONFINITE = -4,  /* NaN/Inf coordinate, or two atoms at the same point */
+  MD_ECUDA = -5,       /* CUDA runtime error, or no device */
+  MD_ESTATE = -6       /* call out of order (e.g. md_get_neighbors before any build) */
+};
+
+/* bits of md_stats.error_flags */
+enum { MD_FLAG_OVERFLOW = 1, MD_FLAG_NONFINITE = 2 };
+
+enum { MD_POT_TBSMA = 0, MD_POT_EAM_TABLE = 1 };
+enum { MD_MAX_TYPES = 4 };
+
+typedef struct md_system md_system; /* opaque; lives in host memory, owned by the library */
+
+typedef struct {
+  int n_atoms, n_boxes, n_types;  /* n_boxes = 1: one box.  > 1: batched mode, n_atoms = total, equal
+                                     atoms per box.  1 <= n_types <= MD_MAX_TYPES.  n_atoms <= 2^26. */
+  double box[3];                  /* orthorhombic edge lengths, all periodic; the same for every box of a batch */
+  double cutoff, skin;            /* r_c and the Verlet skin; the list holds pairs with r < r_c + skin */
+  const double *positions;        /* [n_atoms][3]; any real values (wrapped into the box at every build) */
+  const double *velocities;       /* [n_atoms][3] Angstrom/fs, or NULL (= 0) */
+  const int *types;               /* [n_atoms], each in [0, n_types) */
+  const double *mass;             /* [n_types] amu, HOST */
+  int pot_kind;                   /* MD_POT_TBSMA or MD_POT_EAM_TABLE */
+  /* MD_POT_TBSMA: second-moment tight binding, F(rho) = -sqrt(rho), per type pair
+   * [n_types*n_types], HOST:  rho(r) = xi^2 exp(-2q(r/r0-1)) S(r),  V(r) = 2A exp(-p(r/r0-1)) S(r),
+   * S = quintic switch from 1 at taper_on to 0 at cutoff (taper_on < cutoff). */
+  const double *A, *xi, *p, *q, *r0;
+  double taper_on;
+  /* MD_POT_EAM_TABLE: look-up tables "created once on a CPU and copied to the device".
+   * Uniform grids, node VALUES and node SLOPES; evaluation is the cubic Hermite interpolant and, for the
+   * force, the derivative of that same interpolant.  r_k = k*dr, k < nr, r_{nr-1} >= cutoff;
+   * rho_k = k*drho, k < nrho; above rho_{nrho-1} F continues linearly. */
+  int nr;
+  double dr;
+  const double *f_val, *f_der, *phi_val, *phi_der; /* [n_types*n_types][nr]: rho(r) and V(r) per type pair */
+  int nrho;
+  double drho;
+  const double *F_val, *F_der;                     /* [n_types][nrho] */
+  int max_neighbors;              /* list capacity per atom (the paper's MN); 0 = chosen from the number density */
+  void *stream;                   /* cudaStream_t */
+} md_desc;
+
+typedef struct {
+  long steps, rebuilds;           /* time steps taken; neighbour builds done (explicit and displacement-triggered) */
+  int max_neighbors;              /* largest list length seen at the last build */
+  int error_flags;                /* MD_FLAG_* bits, sticky */
+  double last_max_disp2;          /* max_i |x_i - x_ref,i|^2 at the last displacement check (Angstrom^2) */
+  int neighbor_capacity;          /* list capacity per atom in use */
+} md_stats;
+
+/* Bytes of device workspace md_create needs for this description (pointers in *d are not read). */
+int md_workspace_bytes(const md_desc *d, size_t *bytes);
+
+/* Build a system: copies positions/velocities/types/potential into the workspace (device pointer,
+ * 256-byte aligned, `bytes` >= md_workspace_bytes).  No neighbour list exists yet.  *out is set only on MD_OK.
+ * Errors: MD_EINVAL, MD_EBOX (some L_a < 3 (cutoff+skin)), MD_ECUDA. */
+int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out);
+int md_destroy(md_system *s);
+
+/* Sec. 3.2 / Fig.3 on the device: wrap into the box, cell index, histogram, scan, scatter into cell order
+ * (deterministic: ties inside a cell ordered by caller index), re-order positions/velocities/types, build
+ * the full neighbour list { j != i, same box : |r_ij|^2 < (cutoff+skin)^2 } with the minimum image
+ * d = x_j - x_i; if (d > L/2) d -= L; else if (d < -L/2) d += L; r2 = (dx*dx + dy*dy) + dz*dz, every
+ * operation rounded once (no FMA), and record x_ref <- x.  Invalidates forces. */
+int md_build_neighbors(md_system *s);
+
+/* Fig.5 then Fig.6: densities rho_i and F'(rho_i), then forces (eq.3), per-atom energies (eq.1) and the
+ * virial W^{ab} = 1/2 sum_i sum_j (r_i - r_j)^a f_ij^b per box, components xx,yy,zz,xy,xz,yz.
+ * Builds the list first if there is none or if some atom moved more than skin/2 since the last build.
+ *   forces [n_atoms][3] eV/A, e_atom [n_atoms] eV, virial [n_boxes][6] eV; each may be NULL. */
+int md_compute_forces(md_system *s, double *forces, double *e_atom, double *virial);
+
+/* n velocity-Verlet steps of dt fs:  v += (dt/2m) f;  x += dt v;  if max_i |x_i - x_ref,i|^2 > (skin/2)^2
+ * rebuild (one flag for the whole batch);  f = force(x);  v += (dt/2m) f.  Forces are evaluated once before
+ * the first step if they are stale.  Nothing crosses the host/device boundary inside the call; the rebuild
+ * decision is taken on the device. */
+int md_step(md_system *s, int n, double dt);
+
+int md_get_positions(md_system *s, double *x);        /* [n_atoms][3]; as wrapped at the last build plus drift since */
+int md_get_velocities(md_system *s, double *v);       /* [n_atoms][3] */
+int md_set_positions(md_system *s, const double *x);  /* keeps the list if no atom is farther than skin/2 from x_ref */
+int md_set_velocities(md_system *s, const double *v);
+/* Test hook: the list as ORIGINAL (caller) indices, ascending per atom.  count [n_atoms], list [n_atoms][stride];
+ * MD_ESTATE before the first build, MD_EOVERFLOW if some count exceeds stride. */
+int md_get_neighbors(md_system *s, int *count, int *list, int stride);
+/* Test hook: rho_i and F'(rho_i) of the last force evaluation, [n_atoms] each (either may be NULL). */
+int md_get_densities(md_system *s, double *rho, double *fprime);
+/* Potential and kinetic energy per box, [n_boxes] each (either may be NULL); evaluates forces if stale. Synchronises. */
+int md_get_energies(md_system *s, double *epot, double *ekin);
+int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
+
+/* Options (all default 0):
+ *  MD_OPT_STEP_OBSERVABLES  1: every force evaluation inside md_step also accumulates per-atom energy and the
+ *                              virial (the paper's force kernel with pressure); 0: forces only
+ *                              (the paper's full-MD runs).  md_compute_forces always computes them.
+ *  MD_OPT_PROFILE           1: bracket every kernel launch with CUDA events on the system's stream so that
+ *                              md_profile_read can report per-kernel device time.
+ *  MD_OPT_FORCE_VARIANT     0: choose by neighbour count; 1: thread-per-atom; 2: warp-per-atom. */
+enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3 };
+int md_set_option(md_system *s, int option, int value);
+
+/* Kernel classes for md_profile_read */
+enum { MD_K_BIN = 0, MD_K_SCAN, MD_K_SORT, MD_K_REORDER, MD_K_LIST, MD_K_DENSITY, MD_K_FORCE, MD_K_INTEGRATE,
+       MD_K_REDUCE, MD_K_COUNT };
+/* Sum of CUDA-event elapsed time (ms) and number of launches of one kernel class since the last
+ * md_profile_reset; synchronises.  Needs MD_OPT_PROFILE. */
+int md_profile_read(md_system *s, int kernel_class, long *launches, double *total_ms);
+int md_profile_reset(md_system *s);
+const char *md_kernel_name(int kernel_class);
+
+/* Diagnostic: measured FP64 issue rate of this device, in DFMA thread-instructions per second, from a
+ * register-resident kernel of independent DFMA chains on every SM (the ALU roofline denominator). */
+int md_fp64_dfma_rate(void *stream, double *dfma_per_s, double *sm_clock_mhz);
+
+const char *md_strerror(int status);
+const char *md_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
