@@ -132,8 +132,8 @@ int md_get_positions(md_system *s, double *x);        /* [n_atoms][3]; as wrappe
 int md_get_velocities(md_system *s, double *v);       /* [n_atoms][3] */
 int md_set_positions(md_system *s, const double *x);  /* keeps the list if no atom is farther than skin/2 from x_ref */
 int md_set_velocities(md_system *s, const double *v);
-/* Test hook: the list as ORIGINAL (caller) indices, ascending per atom.  count [n_atoms], list [n_atoms][stride];
- * MD_ESTATE before the first build, MD_EOVERFLOW if some count exceeds stride. */
+/* Test hook: the list as ORIGINAL (caller) indices, ascending per atom.  count [n_atoms], list [n_atoms][stride]
+ * (each row padded with -1); MD_ESTATE before the first build, MD_EOVERFLOW if some count exceeds stride. */
 int md_get_neighbors(md_system *s, int *count, int *list, int stride);
 /* Test hook: rho_i and F'(rho_i) of the last force evaluation, [n_atoms] each (either may be NULL). */
 int md_get_densities(md_system *s, double *rho, double *fprime);

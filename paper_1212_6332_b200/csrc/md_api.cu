@@ -1,0 +1,612 @@
+// md_api.cu — the C ABI of include/md.h: argument checking, workspace layout, host/device staging,
+// and the call sequences of md_build_neighbors / md_compute_forces / md_step.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "md_internal.cuh"
+
+using namespace md;
+
+namespace md {
+
+// ------------------------------------------------------------------------------------------------
+// profiling scopes
+// ------------------------------------------------------------------------------------------------
+ProfScope::ProfScope(md_system *sys, int c) : s(sys), cls(c) {
+  if (!s->opt_profile) return;
+  ProfClass &p = s->prof[cls];
+  if (p.used + 2 > p.ev.size()) {
+    if (p.ev.size() >= 2 * 65536) { p.dropped++; return; }
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { p.dropped++; return; }
+    p.ev.push_back(a); p.ev.push_back(b);
+  }
+  cudaEventRecord(p.ev[p.used], s->stream);
+  stop = p.ev[p.used + 1];
+  p.used += 2;
+}
+ProfScope::~ProfScope() { if (stop) cudaEventRecord(stop, s->stream); }
+
+// ------------------------------------------------------------------------------------------------
+// workspace layout: one bump allocation, 256-byte aligned pieces
+// ------------------------------------------------------------------------------------------------
+struct Bump {
+  char *base; size_t off = 0;
+  explicit Bump(void *b) : base((char *)b) {}
+  template <class T> T *take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T *p = base ? (T *)(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+struct Geometry { int nc[3], tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
+
+static int geometry(const md_desc *d, Geometry &g) {
+  if (!d || d->n_atoms <= 0 || d->n_boxes <= 0 || d->n_types <= 0 || d->n_types > MD_MAX_TYPES) return MD_EINVAL;
+  if (d->n_atoms % d->n_boxes || d->n_atoms > kMaxAtoms) return MD_EINVAL;
+  if (!(d->cutoff > 0.0) || !(d->skin >= 0.0) || !isfinite(d->cutoff) || !isfinite(d->skin)) return MD_EINVAL;
+  if (d->pot_kind != MD_POT_TBSMA && d->pot_kind != MD_POT_EAM_TABLE) return MD_EINVAL;
+  if (d->pot_kind == MD_POT_EAM_TABLE && (d->nr < 2 || d->nrho < 2 || !(d->dr > 0.0) || !(d->drho > 0.0))) return MD_EINVAL;
+  if (d->pot_kind == MD_POT_EAM_TABLE && (double)(d->nr - 1) * d->dr < d->cutoff * (1.0 - 1e-12)) return MD_EINVAL;
+  if (d->pot_kind == MD_POT_TBSMA && !(d->taper_on < d->cutoff)) return MD_EINVAL;
+  if (d->max_neighbors < 0) return MD_EINVAL;
+  const double rl = d->cutoff + d->skin;
+  g.npb = d->n_atoms / d->n_boxes;
+  double vol = 1.0;
+  for (int a = 0; a < 3; ++a) {
+    if (!(d->box[a] > 0.0) || !isfinite(d->box[a])) return MD_EINVAL;
+    g.nc[a] = (int)floor(d->box[a] / rl);
+    if (g.nc[a] < 3) return MD_EBOX;                 // 26 distinct neighbour cells
+    vol *= d->box[a];
+  }
+  const double cells = (double)g.nc[0] * g.nc[1] * g.nc[2];
+  if (cells * d->n_boxes > 1.6e7) return MD_EINVAL;  // two-level scan limit (4096 * 4096 cells)
+  g.tnc = g.nc[0] * g.nc[1] * g.nc[2];
+  g.ncell = g.tnc * d->n_boxes;
+  if (d->max_neighbors > 0) g.cap = d->max_neighbors;
+  else {
+    // MN "adjusted according to the particle density of the system and the cut-off"
+    const double expect = 4.18879020478639 * rl * rl * rl * (double)g.npb / vol;
+    g.cap = (int)(1.5 * expect) + 16;
+  }
+  if (g.cap > g.npb - 1) g.cap = g.npb - 1;
+  if (g.cap < 4) g.cap = 4;
+  g.cap = (g.cap + 3) & ~3;
+  g.tiles_per_box = (g.npb + 31) / 32;
+  g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock);
+  g.stage_bytes = (size_t)d->n_atoms * 3 * sizeof(double);
+  if (g.stage_bytes < (1u << 20)) g.stage_bytes = 1u << 20;
+  return MD_OK;
+}
+
+static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system *sys) {
+  Bump b(base);
+  DevSys t;  // filled only when sys != nullptr
+  const size_t N = (size_t)d->n_atoms, nt2 = (size_t)d->n_types * d->n_types;
+  t.st = b.take<DevState>(1);
+  t.pos = b.take<double4>(N); t.posf = b.take<double4>(N); t.pos_tmp = b.take<double4>(N);
+  t.vel = b.take<double>(3 * N); t.vel_tmp = b.take<double>(3 * N);
+  t.frc = b.take<double>(3 * N); t.xref = b.take<double>(3 * N);
+  t.type = b.take<int>(N); t.type_tmp = b.take<int>(N); t.orig = b.take<int>(N); t.orig_tmp = b.take<int>(N);
+  t.cell_id = b.take<int>(N); t.perm = b.take<int>(N);
+  t.cell_count = b.take<int>((size_t)g.ncell + 1); t.cell_start = b.take<int>((size_t)g.ncell + 1);
+  t.cell_fill = b.take<int>((size_t)g.ncell + 1);
+  t.scan_block = b.take<int>(4096);
+  t.nbr = b.take<unsigned>((size_t)d->n_boxes * g.tiles_per_box * g.cap * 32);
+  t.ncount = b.take<int>(N);
+  t.rho = b.take<double>(N); t.eemb = b.take<double>(N); t.eatom = b.take<double>(N);
+  t.partial = b.take<double>((size_t)g.n_blocks * 8);
+  t.box_epot = b.take<double>(d->n_boxes); t.box_virial = b.take<double>((size_t)d->n_boxes * 6);
+  t.box_ekin = b.take<double>(d->n_boxes);
+  double *tabs[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  if (d->pot_kind == MD_POT_EAM_TABLE) {
+    for (int k = 0; k < 4; ++k) tabs[k] = b.take<double>(nt2 * d->nr);
+    for (int k = 4; k < 6; ++k) tabs[k] = b.take<double>((size_t)d->n_types * d->nrho);
+  }
+  void *stage = b.take<char>(g.stage_bytes);
+  if (sys) {
+    DevSys &o = sys->d;
+    o.st = t.st; o.pos = t.pos; o.posf = t.posf; o.pos_tmp = t.pos_tmp; o.vel = t.vel; o.vel_tmp = t.vel_tmp;
+    o.frc = t.frc; o.xref = t.xref; o.type = t.type; o.type_tmp = t.type_tmp; o.orig = t.orig; o.orig_tmp = t.orig_tmp;
+    o.cell_id = t.cell_id; o.perm = t.perm; o.cell_count = t.cell_count; o.cell_start = t.cell_start;
+    o.cell_fill = t.cell_fill; o.scan_block = t.scan_block; o.nbr = t.nbr; o.ncount = t.ncount; o.rho = t.rho;
+    o.eemb = t.eemb; o.eatom = t.eatom; o.partial = t.partial; o.box_epot = t.box_epot; o.box_virial = t.box_virial;
+    o.box_ekin = t.box_ekin;
+    o.tab.f_val = tabs[0]; o.tab.f_der = tabs[1]; o.tab.phi_val = tabs[2]; o.tab.phi_der = tabs[3];
+    o.tab.F_val = tabs[4]; o.tab.F_der = tabs[5];
+    sys->stage = stage; sys->stage_bytes = g.stage_bytes;
+  }
+  return (b.off + 255) & ~(size_t)255;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host / device pointer handling
+// ------------------------------------------------------------------------------------------------
+static bool on_device(const void *p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// ---- conversion kernels between caller order (AoS [N][3]) and cell order ------------------------
+__global__ void k_init_atoms(const __grid_constant__ DevSys s, const double *__restrict__ x, const int *__restrict__ types) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const int t = types[i];
+  if (t < 0 || t >= s.nt) atomicOr(&s.st->error_flags, 1 << 30);
+  s.pos[i] = make_double4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], (double)t);
+  s.type[i] = t;
+  s.orig[i] = i;
+}
+
+__global__ void k_set_vec(const __grid_constant__ DevSys s, double *__restrict__ dst, const double *__restrict__ src) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;   // slot
+  if (i >= s.N) return;
+  const size_t o = 3 * (size_t)s.orig[i];
+  dst[i] = src ? src[o] : 0.0; dst[(size_t)s.N + i] = src ? src[o + 1] : 0.0; dst[2 * (size_t)s.N + i] = src ? src[o + 2] : 0.0;
+}
+
+__global__ void k_get_vec(const __grid_constant__ DevSys s, const double *__restrict__ src, double *__restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const size_t o = 3 * (size_t)s.orig[i];
+  dst[o] = src[i]; dst[o + 1] = src[(size_t)s.N + i]; dst[o + 2] = src[2 * (size_t)s.N + i];
+}
+
+__global__ void k_get_scalar(const __grid_constant__ DevSys s, const double *__restrict__ src, double *__restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < s.N) dst[s.orig[i]] = src[i];
+}
+
+__global__ void k_get_fprime(const __grid_constant__ DevSys s, double *__restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < s.N) dst[s.orig[i]] = s.posf[i].w;
+}
+
+__global__ void k_get_pos(const __grid_constant__ DevSys s, double *__restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const double4 p = s.pos[i];
+  const size_t o = 3 * (size_t)s.orig[i];
+  dst[o] = p.x; dst[o + 1] = p.y; dst[o + 2] = p.z;
+}
+
+// new positions: take the periodic image nearest x_ref (so that x - x_ref needs no image logic later) and
+// fold the displacement into the rebuild decision
+__global__ void k_set_pos(const __grid_constant__ DevSys s, const double *__restrict__ src, int have_ref) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const size_t o = 3 * (size_t)s.orig[i], N = (size_t)s.N;
+  double4 p = s.pos[i];
+  double x[3] = {src[o], src[o + 1], src[o + 2]};
+  if (have_ref) {
+    double d2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double ref = s.xref[c * N + i];
+      double u = x[c] - ref;
+      u -= s.L[c] * rint(u / s.L[c]);
+      x[c] = ref + u;
+      d2 += u * u;
+    }
+    if (!(d2 == d2)) d2 = __longlong_as_double(0x7ff0000000000000ll);
+    atomicMax(&s.st->maxd2_bits, (unsigned long long)__double_as_longlong(d2));
+  }
+  p.x = x[0]; p.y = x[1]; p.z = x[2];
+  s.pos[i] = p;
+}
+
+// neighbour list as caller indices, ascending per atom (test hook).  perm[] (free outside the rebuild chain)
+// is first filled with the inverse of orig[]; then one thread per CALLER atom in [first, first+natoms)
+// writes its count and its row (insertion sort in place) at chunk-relative position a.
+__global__ void k_invert_orig(const __grid_constant__ DevSys s) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < s.N) s.perm[s.orig[i]] = i;
+}
+
+__global__ void k_export_neighbors(const __grid_constant__ DevSys s, int first, int natoms, int *__restrict__ count,
+                                   int *__restrict__ list, int stride, int *overflow) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= natoms) return;
+  const int i = s.perm[first + a];
+  const int box = i / s.npb, local = i - box * s.npb;
+  const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
+  const unsigned *row = s.nbr + tile * s.cap * 32 + (local & 31);
+  const int n = s.ncount[i];
+  count[a] = n;
+  if (n > stride) { atomicOr(overflow, 1); return; }
+  int *out = list + (size_t)a * stride;
+  for (int k = 0; k < n; ++k) {
+    const int v = s.orig[row[(size_t)k * 32] & kIdxMask];
+    int b = k - 1;
+    while (b >= 0 && out[b] > v) { out[b + 1] = out[b]; --b; }
+    out[b + 1] = v;
+  }
+  for (int k = n; k < stride; ++k) out[k] = -1;      // rows are padded with -1
+}
+
+static inline int grid_for(int n, int tb = 256) { return (n + tb - 1) / tb; }
+
+static int check_cuda(cudaError_t e) { return e == cudaSuccess ? MD_OK : MD_ECUDA; }
+
+static int sync_and_flags(md_system *s, int *flags_out = nullptr) {
+  DevState st;
+  if (cudaMemcpyAsync(&st, s->d.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  if (flags_out) *flags_out = st.error_flags;
+  if (st.error_flags & MD_FLAG_NONFINITE) return MD_ENONFINITE;
+  if (st.error_flags & MD_FLAG_OVERFLOW) return MD_EOVERFLOW;
+  return MD_OK;
+}
+
+// copy `bytes` from a device scratch/result buffer to a user pointer (host or device)
+static int deliver(md_system *s, void *user, const void *dev, size_t bytes, bool *was_host) {
+  const bool dev_ptr = on_device(user);
+  if (was_host) *was_host = !dev_ptr;
+  return check_cuda(cudaMemcpyAsync(user, dev, bytes, dev_ptr ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+}
+
+static int forces_sequence(md_system *s, bool observables, double half_dt) {
+  int rc;
+  if ((rc = launch_rebuild_chain(s)) != 0) return MD_ECUDA;
+  if ((rc = launch_density(s)) != 0) return MD_ECUDA;
+  if ((rc = launch_force(s, observables, half_dt)) != 0) return MD_ECUDA;
+  s->have_list = true;
+  s->forces_valid = true;
+  s->observables_valid = observables;
+  return MD_OK;
+}
+
+static int request_rebuild(md_system *s) {
+  const int one = 1;
+  return check_cuda(cudaMemcpyAsync(&s->d.st->force_rebuild, &one, sizeof(int), cudaMemcpyHostToDevice, s->stream));
+}
+
+}  // namespace md
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+extern "C" {
+
+const char *md_strerror(int e) {
+  switch (e) {
+    case MD_OK: return "ok";
+    case MD_EINVAL: return "invalid argument";
+    case MD_EBOX: return "box edge shorter than 3 (cutoff + skin)";
+    case MD_EOVERFLOW: return "neighbour-list capacity exceeded";
+    case MD_ENONFINITE: return "non-finite coordinate or coincident atoms";
+    case MD_ECUDA: return "CUDA error or no device";
+    case MD_ESTATE: return "call out of order";
+  }
+  return "unknown status";
+}
+
+const char *md_version(void) { return "paper_1212_6332_b200 0.1 (sm_100a)"; }
+
+const char *md_kernel_name(int c) {
+  static const char *names[MD_K_COUNT] = {"bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce"};
+  return (c >= 0 && c < MD_K_COUNT) ? names[c] : "?";
+}
+
+int md_workspace_bytes(const md_desc *d, size_t *bytes) {
+  Geometry g;
+  int rc = geometry(d, g);
+  if (rc != MD_OK) return rc;
+  if (!bytes) return MD_EINVAL;
+  *bytes = layout(d, g, nullptr, nullptr);
+  return MD_OK;
+}
+
+int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) {
+  Geometry g;
+  int rc = geometry(d, g);
+  if (rc != MD_OK) return rc;
+  if (!out || !workspace || !d->positions || !d->types || !d->mass) return MD_EINVAL;
+  if (((uintptr_t)workspace & 255) || bytes < layout(d, g, nullptr, nullptr)) return MD_EINVAL;
+  if (!on_device(workspace)) return cudaGetLastError() == cudaSuccess ? MD_EINVAL : MD_ECUDA;
+  if (d->pot_kind == MD_POT_TBSMA && (!d->A || !d->xi || !d->p || !d->q || !d->r0)) return MD_EINVAL;
+  if (d->pot_kind == MD_POT_EAM_TABLE && (!d->f_val || !d->f_der || !d->phi_val || !d->phi_der || !d->F_val || !d->F_der))
+    return MD_EINVAL;
+  for (int t = 0; t < d->n_types; ++t) if (!(d->mass[t] > 0.0) || !isfinite(d->mass[t])) return MD_EINVAL;
+
+  md_system *s = new (std::nothrow) md_system();
+  if (!s) return MD_EINVAL;
+  memset(&s->d, 0, sizeof(s->d));
+  s->stream = (cudaStream_t)d->stream;
+  s->cutoff = d->cutoff; s->skin = d->skin;
+  s->have_list = s->forces_valid = s->observables_valid = false;
+  s->opt_step_obs = s->opt_profile = false; s->opt_force_variant = 0; s->steps = 0;
+  layout(d, g, workspace, s);
+  DevSys &o = s->d;
+  o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
+  const double rl = d->cutoff + d->skin;
+  for (int a = 0; a < 3; ++a) {
+    o.L[a] = d->box[a]; o.hL[a] = 0.5 * d->box[a]; o.nc[a] = g.nc[a]; o.cell_scale[a] = (double)g.nc[a] / d->box[a];
+  }
+  o.rc2 = d->cutoff * d->cutoff; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
+  o.tnc = g.tnc; o.ncell = g.ncell; o.cap = g.cap; o.tiles_per_box = g.tiles_per_box;
+  s->n_force_blocks = g.n_blocks;
+  for (int t = 0; t < d->n_types; ++t) s->mass_ev[t] = d->mass[t] * kAmuToEvFs2PerA2;
+  const size_t N = (size_t)o.N, nt2 = (size_t)o.nt * o.nt;
+  cudaStream_t st = s->stream;
+  cudaError_t e = cudaMemsetAsync(o.st, 0, sizeof(DevState), st);
+  if (d->pot_kind == MD_POT_TBSMA) {
+    for (size_t k = 0; k < nt2; ++k) {
+      if (!(d->r0[k] > 0.0)) { delete s; return MD_EINVAL; }
+      o.tb.A2[k] = 2.0 * d->A[k]; o.tb.xi2[k] = d->xi[k] * d->xi[k];
+      o.tb.p[k] = d->p[k]; o.tb.p_r0[k] = d->p[k] / d->r0[k];
+      o.tb.q2[k] = 2.0 * d->q[k]; o.tb.q2_r0[k] = 2.0 * d->q[k] / d->r0[k];
+    }
+    o.tb.r_on = d->taper_on; o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on);
+  } else {
+    TableParams &t = o.tab;
+    t.nr = d->nr; t.nrho = d->nrho; t.dr = d->dr; t.inv_dr = 1.0 / d->dr; t.drho = d->drho; t.inv_drho = 1.0 / d->drho;
+    t.rho_max = (double)(d->nrho - 1) * d->drho;
+    const void *src[6] = {d->f_val, d->f_der, d->phi_val, d->phi_der, d->F_val, d->F_der};
+    void *dst[6] = {(void *)t.f_val, (void *)t.f_der, (void *)t.phi_val, (void *)t.phi_der, (void *)t.F_val, (void *)t.F_der};
+    for (int k = 0; k < 6 && e == cudaSuccess; ++k)
+      e = cudaMemcpyAsync(dst[k], src[k], (k < 4 ? nt2 * d->nr : (size_t)o.nt * d->nrho) * sizeof(double), cudaMemcpyDefault, st);
+  }
+  // positions + types (through the staging area when they live on the host)
+  const double *xdev = d->positions;
+  const int *tdev = d->types;
+  if (e == cudaSuccess && !on_device(d->positions)) {
+    e = cudaMemcpyAsync(s->stage, d->positions, 3 * N * sizeof(double), cudaMemcpyHostToDevice, st);
+    xdev = (const double *)s->stage;
+  }
+  if (e == cudaSuccess && !on_device(d->types)) {
+    e = cudaMemcpyAsync(o.cell_id, d->types, N * sizeof(int), cudaMemcpyHostToDevice, st);   // cell_id is free before the first build
+    tdev = o.cell_id;
+  }
+  if (e == cudaSuccess) {
+    k_init_atoms<<<grid_for(o.N), 256, 0, st>>>(o, xdev, tdev);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) {
+    const double *vdev = d->velocities;
+    if (vdev && !on_device(vdev)) {
+      e = cudaMemcpyAsync(s->stage, vdev, 3 * N * sizeof(double), cudaMemcpyHostToDevice, st);   // stream order: after k_init_atoms
+      vdev = (const double *)s->stage;
+    }
+    if (e == cudaSuccess) { k_set_vec<<<grid_for(o.N), 256, 0, st>>>(o, o.vel, vdev); e = cudaGetLastError(); }
+  }
+  if (e == cudaSuccess) e = cudaMemsetAsync(o.frc, 0, 3 * N * sizeof(double), st);
+  int flags = 0;
+  if (e != cudaSuccess || sync_and_flags(s, &flags) == MD_ECUDA) { delete s; cudaGetLastError(); return MD_ECUDA; }
+  if (flags & (1 << 30)) { delete s; return MD_EINVAL; }   // a type out of range
+  *out = s;
+  return MD_OK;
+}
+
+int md_destroy(md_system *s) {
+  if (!s) return MD_OK;
+  cudaStreamSynchronize(s->stream);
+  for (auto &p : s->prof) for (cudaEvent_t ev : p.ev) cudaEventDestroy(ev);
+  delete s;
+  return MD_OK;
+}
+
+int md_set_option(md_system *s, int option, int value) {
+  if (!s) return MD_EINVAL;
+  switch (option) {
+    case MD_OPT_STEP_OBSERVABLES: s->opt_step_obs = value != 0; return MD_OK;
+    case MD_OPT_PROFILE: s->opt_profile = value != 0; return MD_OK;
+    case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; return MD_OK;
+  }
+  return MD_EINVAL;
+}
+
+int md_build_neighbors(md_system *s) {
+  if (!s) return MD_EINVAL;
+  int rc = request_rebuild(s);
+  if (rc != MD_OK) return rc;
+  if (launch_rebuild_chain(s) != 0) return MD_ECUDA;
+  s->have_list = true; s->forces_valid = false; s->observables_valid = false;
+  return MD_OK;
+}
+
+int md_compute_forces(md_system *s, double *forces, double *e_atom, double *virial) {
+  if (!s) return MD_EINVAL;
+  int rc;
+  if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+  if ((rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+  const DevSys &o = s->d;
+  bool any_host = false, h;
+  double *scratch = (double *)s->stage;
+  if (forces) {
+    if (on_device(forces)) k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, forces);
+    else {
+      k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, scratch);
+      if ((rc = deliver(s, forces, scratch, 3 * (size_t)o.N * sizeof(double), &h)) != MD_OK) return rc;
+      any_host = true;
+    }
+  }
+  if (e_atom) {
+    if (on_device(e_atom)) k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, e_atom);
+    else {
+      k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, scratch);   // stream order: after the copy above
+      if ((rc = deliver(s, e_atom, scratch, (size_t)o.N * sizeof(double), &h)) != MD_OK) return rc;
+      any_host = true;
+    }
+  }
+  if (virial) {
+    if ((rc = deliver(s, virial, o.box_virial, 6 * (size_t)o.nb * sizeof(double), &h)) != MD_OK) return rc;
+    any_host |= h;
+  }
+  if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
+  return any_host ? sync_and_flags(s) : MD_OK;
+}
+
+int md_step(md_system *s, int n, double dt) {
+  if (!s || n < 0 || !isfinite(dt)) return MD_EINVAL;
+  int rc;
+  if (n == 0) return MD_OK;
+  if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+  if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
+  for (int k = 0; k < n; ++k) {
+    if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
+    if ((rc = forces_sequence(s, s->opt_step_obs, 0.5 * dt)) != MD_OK) return rc;
+  }
+  s->steps += n;
+  return MD_OK;
+}
+
+int md_get_positions(md_system *s, double *x) {
+  if (!s || !x) return MD_EINVAL;
+  const DevSys &o = s->d;
+  if (on_device(x)) { k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, x); return check_cuda(cudaGetLastError()); }
+  k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, (double *)s->stage);
+  int rc = deliver(s, x, s->stage, 3 * (size_t)o.N * sizeof(double), nullptr);
+  return rc != MD_OK ? rc : sync_and_flags(s);
+}
+
+int md_get_velocities(md_system *s, double *v) {
+  if (!s || !v) return MD_EINVAL;
+  const DevSys &o = s->d;
+  if (on_device(v)) { k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, v); return check_cuda(cudaGetLastError()); }
+  k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, (double *)s->stage);
+  int rc = deliver(s, v, s->stage, 3 * (size_t)o.N * sizeof(double), nullptr);
+  return rc != MD_OK ? rc : sync_and_flags(s);
+}
+
+int md_set_positions(md_system *s, const double *x) {
+  if (!s || !x) return MD_EINVAL;
+  const DevSys &o = s->d;
+  const double *src = x;
+  if (!on_device(x)) {
+    if (cudaMemcpyAsync(s->stage, x, 3 * (size_t)o.N * sizeof(double), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
+    src = (const double *)s->stage;
+  }
+  k_set_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, src, s->have_list ? 1 : 0);
+  s->forces_valid = false; s->observables_valid = false;
+  if (src != x && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;   // the host buffer may be reused
+  return check_cuda(cudaGetLastError());
+}
+
+int md_set_velocities(md_system *s, const double *v) {
+  if (!s || !v) return MD_EINVAL;
+  const DevSys &o = s->d;
+  const double *src = v;
+  if (!on_device(v)) {
+    if (cudaMemcpyAsync(s->stage, v, 3 * (size_t)o.N * sizeof(double), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
+    src = (const double *)s->stage;
+  }
+  k_set_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, src);
+  if (src != v && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  return check_cuda(cudaGetLastError());
+}
+
+int md_get_neighbors(md_system *s, int *count, int *list, int stride) {
+  if (!s || !count || !list || stride <= 0) return MD_EINVAL;
+  if (!s->have_list) return MD_ESTATE;
+  const DevSys &o = s->d;
+  const bool dev = on_device(list);
+  if (dev != on_device(count)) return MD_EINVAL;       // both on the same side
+  int *flag = o.scan_block;                            // free outside the rebuild chain
+  if (cudaMemsetAsync(flag, 0, sizeof(int), s->stream) != cudaSuccess) return MD_ECUDA;
+  k_invert_orig<<<grid_for(o.N), 256, 0, s->stream>>>(o);
+  if (dev) {
+    k_export_neighbors<<<grid_for(o.N, 128), 128, 0, s->stream>>>(o, 0, o.N, count, list, stride, flag);
+  } else {
+    // chunks of caller atoms that fit the staging area: [chunk] counts followed by [chunk][stride] rows
+    const size_t per_atom = ((size_t)stride + 1) * sizeof(int);
+    const int chunk = (int)(s->stage_bytes / per_atom < (size_t)o.N ? s->stage_bytes / per_atom : (size_t)o.N);
+    if (chunk < 1) return MD_EINVAL;
+    int *dcount = (int *)s->stage, *dlist = dcount + chunk;
+    for (int first = 0; first < o.N; first += chunk) {
+      const int na = o.N - first < chunk ? o.N - first : chunk;
+      k_export_neighbors<<<grid_for(na, 128), 128, 0, s->stream>>>(o, first, na, dcount, dlist, stride, flag);
+      if (cudaMemcpyAsync(count + first, dcount, (size_t)na * sizeof(int), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+          cudaMemcpyAsync(list + (size_t)first * stride, dlist, (size_t)na * stride * sizeof(int), cudaMemcpyDeviceToHost,
+                          s->stream) != cudaSuccess)
+        return MD_ECUDA;
+    }
+  }
+  int over = 0;
+  if (cudaMemcpyAsync(&over, flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  int rc = sync_and_flags(s);
+  if (rc != MD_OK) return rc;
+  return over ? MD_EOVERFLOW : MD_OK;
+}
+
+int md_get_densities(md_system *s, double *rho, double *fprime) {
+  if (!s) return MD_EINVAL;
+  if (!s->forces_valid) return MD_ESTATE;
+  const DevSys &o = s->d;
+  int rc;
+  bool any_host = false;
+  double *scratch = (double *)s->stage;
+  if (rho) {
+    if (on_device(rho)) k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, rho);
+    else {
+      k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, scratch);
+      if ((rc = deliver(s, rho, scratch, (size_t)o.N * sizeof(double), nullptr)) != MD_OK) return rc;
+      any_host = true;
+    }
+  }
+  if (fprime) {
+    if (on_device(fprime)) k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, fprime);
+    else {
+      k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, scratch);
+      if ((rc = deliver(s, fprime, scratch, (size_t)o.N * sizeof(double), nullptr)) != MD_OK) return rc;
+      any_host = true;
+    }
+  }
+  if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
+  return any_host ? sync_and_flags(s) : MD_OK;
+}
+
+int md_get_energies(md_system *s, double *epot, double *ekin) {
+  if (!s) return MD_EINVAL;
+  int rc;
+  const DevSys &o = s->d;
+  if (epot) {
+    if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+    if (!(s->forces_valid && s->observables_valid) && (rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+    if ((rc = deliver(s, epot, o.box_epot, (size_t)o.nb * sizeof(double), nullptr)) != MD_OK) return rc;
+  }
+  if (ekin) {
+    if (launch_ekin(s) != 0) return MD_ECUDA;
+    if ((rc = deliver(s, ekin, o.box_ekin, (size_t)o.nb * sizeof(double), nullptr)) != MD_OK) return rc;
+  }
+  return sync_and_flags(s);
+}
+
+int md_get_stats(md_system *s, md_stats *out) {
+  if (!s || !out) return MD_EINVAL;
+  DevState st;
+  if (cudaMemcpyAsync(&st, s->d.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  out->steps = s->steps; out->rebuilds = (long)st.rebuilds; out->max_neighbors = st.max_neighbors;
+  out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap;
+  return MD_OK;
+}
+
+int md_profile_reset(md_system *s) {
+  if (!s) return MD_EINVAL;
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  for (auto &p : s->prof) { p.used = 0; p.dropped = 0; }
+  return MD_OK;
+}
+
+int md_profile_read(md_system *s, int cls, long *launches, double *total_ms) {
+  if (!s || cls < 0 || cls >= MD_K_COUNT) return MD_EINVAL;
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  const ProfClass &p = s->prof[cls];
+  double tot = 0.0;
+  for (size_t k = 0; k + 1 < p.used; k += 2) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, p.ev[k], p.ev[k + 1]) != cudaSuccess) return MD_ECUDA;
+    tot += ms;
+  }
+  if (launches) *launches = (long)(p.used / 2);
+  if (total_ms) *total_ms = tot;
+  return MD_OK;
+}
+
+}  // extern "C"

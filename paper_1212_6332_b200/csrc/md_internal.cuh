@@ -1,0 +1,110 @@
+// md_internal.cuh — internal types shared by the translation units of libmd_b200.so.
+// Nothing here is visible across the C ABI (include/md.h) and nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/md.h"
+
+namespace md {
+
+constexpr int kIdxBits = 26;                       // neighbour entry = index | (image code << 26)
+constexpr unsigned kIdxMask = (1u << kIdxBits) - 1u;
+constexpr int kMaxAtoms = 1 << kIdxBits;
+constexpr int kPairs = MD_MAX_TYPES * MD_MAX_TYPES;
+constexpr double kAmuToEvFs2PerA2 = 103.642696526805;  // 1 amu (A/fs)^2 in eV
+
+// Device-resident mutable state (one per system).
+struct DevState {
+  unsigned long long maxd2_bits;   // bit pattern of max_i |x_i - x_ref,i|^2 since the last check (>=0 doubles order as u64)
+  double last_maxd2;               // value consumed by the last rebuild decision
+  int force_rebuild;               // host request: rebuild at the next decision point
+  int do_rebuild;                  // decision of the current rebuild chain
+  int error_flags;                 // MD_FLAG_* (sticky)
+  int max_neighbors;               // of the last build
+  unsigned long long rebuilds;
+};
+
+struct TbsmaParams {               // per type pair, pre-combined on the host
+  double A2[kPairs];               // 2A
+  double xi2[kPairs];              // xi^2
+  double p[kPairs], p_r0[kPairs];  // p, p/r0
+  double q2[kPairs], q2_r0[kPairs];// 2q, 2q/r0
+  double r_on, inv_w;              // taper start, 1/(r_c - r_on)
+};
+
+struct TableParams {
+  int nr, nrho;
+  double dr, inv_dr, drho, inv_drho, rho_max;
+  const double *f_val, *f_der, *phi_val, *phi_der;   // [nt*nt][nr]
+  const double *F_val, *F_der;                       // [nt][nrho]
+};
+
+// Everything a kernel needs, passed by value as a __grid_constant__ parameter.
+struct DevSys {
+  int N, nb, npb, nt;
+  double L[3], hL[3];
+  double rc2, rl2, thr2;
+  int nc[3], tnc, ncell;           // cells per box (per dim, total) and cells of all boxes
+  double cell_scale[3];            // nc/L
+  int cap;                         // neighbour capacity per atom
+  int tiles_per_box;               // 32-atom tiles per box
+  int kind;
+  // per-atom state, CELL ORDER (index = "slot")
+  double4 *pos;                    // x,y,z, w = type as double
+  double4 *posf;                   // x,y,z, w = F'(rho): written by the density pass, gathered by the force pass
+  double *vel, *frc, *xref;        // SoA, component c at [c*N + i]
+  int *type, *orig;                // orig = caller index of the atom in this slot (paper's hGID)
+  // re-order scratch
+  double4 *pos_tmp; double *vel_tmp; int *type_tmp, *orig_tmp;
+  int *cell_id, *cell_count, *cell_start, *cell_fill, *perm, *scan_block;
+  // neighbour list, blocked ELL: entry k of the atom in (tile, lane) at nbr[(tile*cap + k)*32 + lane]
+  unsigned *nbr; int *ncount;
+  // per-atom results
+  double *rho, *eemb, *eatom;
+  double *partial;                 // [n_blocks][8] block partial sums: E, Wxx,Wyy,Wzz,Wxy,Wxz,Wyz, (pad)
+  double *box_epot, *box_virial, *box_ekin;
+  DevState *st;
+  TbsmaParams tb;
+  TableParams tab;
+};
+
+struct ProfClass { std::vector<cudaEvent_t> ev; size_t used = 0; long dropped = 0; };
+
+}  // namespace md
+
+struct md_system {
+  md::DevSys d;
+  cudaStream_t stream;
+  double mass_ev[MD_MAX_TYPES];    // eV fs^2 / A^2
+  double cutoff, skin;
+  bool have_list, forces_valid, observables_valid;
+  bool opt_step_obs, opt_profile;
+  int opt_force_variant;
+  long steps;
+  void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
+  int n_force_blocks;
+  md::ProfClass prof[MD_K_COUNT];
+};
+
+namespace md {
+// launch geometry of the per-atom kernels that use the tile mapping
+constexpr int kForceBlock = 128;
+inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block; }
+
+// launchers (each enqueues on s->stream; returns cudaError_t of the launch)
+int launch_rebuild_chain(md_system *s);                       // conditional on DevState (force_rebuild / maxd2)
+int launch_density(md_system *s);
+int launch_force(md_system *s, bool observables, double half_dt); // half_dt = dt/2 (0: no velocity update)
+int launch_kick_drift(md_system *s, double dt);
+int launch_reduce_boxes(md_system *s);
+int launch_ekin(md_system *s);
+
+struct ProfScope {                 // brackets launches of one kernel class with events when profiling is on
+  md_system *s; int cls; cudaEvent_t stop = nullptr;
+  ProfScope(md_system *s, int cls);
+  ~ProfScope();
+};
+}  // namespace md

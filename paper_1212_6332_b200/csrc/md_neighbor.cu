@@ -1,0 +1,274 @@
+// md_neighbor.cu — device-side system partitioning and neighbour-list build.
+//
+// Paper: section 3.2 and Fig.3.  The paper computes only the
+// cell index on the GPU (G1-G3) and builds linked lists, sorts atoms by cell and re-sorts velocities
+// on the HOST ("due to its sequential nature").  Here the whole chain runs on the
+// device: histogram -> scan -> scatter -> per-cell ordering -> re-order -> list, and every kernel of the
+// chain is launched unconditionally but returns at once unless DevState says a rebuild is due, so that
+// md_step never needs the host to look at the displacement flag.
+#include "md_internal.cuh"
+
+namespace md {
+
+__device__ __forceinline__ double wrap_coord(double x, double L) {
+  // x - L*floor(x/L), each operation rounded once (same expression as the oracle's wrap)
+  return __dsub_rn(x, __dmul_rn(L, floor(__ddiv_rn(x, L))));
+}
+
+__device__ __forceinline__ int cell_coord(double x, double scale, int nc) {
+  int c = (int)(x * scale);
+  return max(0, min(c, nc - 1));
+}
+
+// ---- K0: decision + clear the cell counters ---------------------------------------------------
+__global__ void k_rebuild_begin(const __grid_constant__ DevSys s, unsigned long long thr2_bits) {
+  const DevState *st = s.st;
+  const bool go = st->force_rebuild != 0 || st->maxd2_bits > thr2_bits;
+  const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (go)
+    for (int c = gid; c <= s.ncell; c += gridDim.x * blockDim.x) { s.cell_count[c] = 0; s.cell_fill[c] = 0; }
+  if (gid == 0) {
+    s.st->do_rebuild = go ? 1 : 0;
+    s.st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
+    if (go) s.st->max_neighbors = 0;
+  }
+}
+
+// ---- K1: wrap, cell index (paper's dIC, G1-G3), histogram (paper's hNAC) ---------------------
+__global__ void k_bin(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  double4 p = s.pos[i];
+  if (!(isfinite(p.x) && isfinite(p.y) && isfinite(p.z))) {
+    atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
+    p.x = p.y = p.z = 0.0;
+  }
+  p.x = wrap_coord(p.x, s.L[0]);
+  p.y = wrap_coord(p.y, s.L[1]);
+  p.z = wrap_coord(p.z, s.L[2]);
+  s.pos[i] = p;
+  const int cx = cell_coord(p.x, s.cell_scale[0], s.nc[0]);
+  const int cy = cell_coord(p.y, s.cell_scale[1], s.nc[1]);
+  const int cz = cell_coord(p.z, s.cell_scale[2], s.nc[2]);
+  // multiple boxes: cell ids of box I shifted by I*TNC
+  const int cid = (i / s.npb) * s.tnc + (cx * s.nc[1] + cy) * s.nc[2] + cz;
+  s.cell_id[i] = cid;
+  atomicAdd(&s.cell_count[cid], 1);
+}
+
+// ---- K2-K4: exclusive scan of cell_count[0..ncell] -> cell_start (paper's hFA) ---------------
+constexpr int kScanThreads = 1024, kScanItems = 4, kScanTile = kScanThreads * kScanItems;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int *total) {
+  __shared__ int warp_sum[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) warp_sum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    int w = warp_sum[lane], winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += t;
+    }
+    warp_sum[lane] = winc - w;          // exclusive prefix of warp totals
+    if (lane == 31) *total = winc;
+  }
+  __syncthreads();
+  return warp_sum[wid] + inc - v;
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_local(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  __shared__ int total;
+  const int n = s.ncell + 1, base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+  int v[kScanItems], sum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) { v[k] = (base + k < n) ? s.cell_count[base + k] : 0; sum += v[k]; }
+  int ex = block_exclusive_scan(sum, &total);
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) { if (base + k < n) s.cell_start[base + k] = ex; ex += v[k]; }
+  if (threadIdx.x == 0) s.scan_block[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_blocks(const __grid_constant__ DevSys s, int nblk) {
+  if (!s.st->do_rebuild) return;
+  __shared__ int total;
+  const int base = threadIdx.x * kScanItems;
+  int v[kScanItems], sum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) { v[k] = (base + k < nblk) ? s.scan_block[base + k] : 0; sum += v[k]; }
+  int ex = block_exclusive_scan(sum, &total);
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) { if (base + k < nblk) s.scan_block[base + k] = ex; ex += v[k]; }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_add(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int n = s.ncell + 1, base = blockIdx.x * kScanTile + threadIdx.x * kScanItems, off = s.scan_block[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) if (base + k < n) s.cell_start[base + k] += off;
+}
+
+// ---- K5: scatter slot indices into their cell segment (order inside a cell not yet defined) ----
+__global__ void k_scatter(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const int c = s.cell_id[i];
+  s.perm[s.cell_start[c] + atomicAdd(&s.cell_fill[c], 1)] = i;
+}
+
+// ---- K6: make the order inside every cell deterministic: ascending caller index -----------------
+__global__ void k_cell_sort(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= s.ncell) return;
+  int *seg = s.perm + s.cell_start[c];
+  const int n = s.cell_count[c];
+  for (int a = 1; a < n; ++a) {
+    const int v = seg[a], key = s.orig[v];
+    int b = a - 1;
+    while (b >= 0 && s.orig[seg[b]] > key) { seg[b + 1] = seg[b]; --b; }
+    seg[b + 1] = v;
+  }
+}
+
+// ---- K7/K8: move every per-atom array into cell order (paper's H9-H28, on the host there) ------
+__global__ void k_reorder(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const int src = s.perm[i];
+  s.pos_tmp[i] = s.pos[src];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) s.vel_tmp[(size_t)c * s.N + i] = s.vel[(size_t)c * s.N + src];
+  s.type_tmp[i] = s.type[src];
+  s.orig_tmp[i] = s.orig[src];
+}
+
+__global__ void k_copyback(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const double4 p = s.pos_tmp[i];
+  s.pos[i] = p;
+  s.xref[i] = p.x; s.xref[(size_t)s.N + i] = p.y; s.xref[2 * (size_t)s.N + i] = p.z;   // x_ref <- x
+#pragma unroll
+  for (int c = 0; c < 3; ++c) s.vel[(size_t)c * s.N + i] = s.vel_tmp[(size_t)c * s.N + i];
+  s.type[i] = s.type_tmp[i];
+  s.orig[i] = s.orig_tmp[i];
+}
+
+// ---- K9: the neighbour list (paper's G6, Fig.3) ---------------------------------------------------
+// One thread per atom (as G6), but no shared-memory tiles: atoms are already in cell order, so the
+// candidates of the three z-adjacent cells of one (x,y) column are one contiguous run of slots.
+// The pair test is the canonical minimum image + non-contracted r2, so the sets are bit-exact.
+// Each entry records which image was taken (2 bits per axis) so that the density and force passes
+// can form the SAME d = (x_j - x_i) -/+ L without re-deciding.
+__device__ __forceinline__ double min_image(double d, double L, double hL, unsigned &code) {
+  code = 0;
+  if (d > hL) { d = __dsub_rn(d, L); code = 2; }          // took  d - L
+  else if (d < -hL) { d = __dadd_rn(d, L); code = 1; }    // took  d + L
+  return d;
+}
+
+__global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
+  const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * blockDim.x + threadIdx.x;
+  if (local >= s.npb) return;
+  const int i = box * s.npb + local;
+  const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
+  unsigned *row = s.nbr + tile * s.cap * 32 + (local & 31);
+  const double4 pi = s.pos[i];
+  const int cx = cell_coord(pi.x, s.cell_scale[0], s.nc[0]);
+  const int cy = cell_coord(pi.y, s.cell_scale[1], s.nc[1]);
+  const int cz = cell_coord(pi.z, s.cell_scale[2], s.nc[2]);
+  const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
+  const int zlo = max(cz - 1, 0), zhi = min(cz + 1, ncz - 1);
+  int n = 0;
+  for (int ox = -1; ox <= 1; ++ox) {
+    int jx = cx + ox; jx += (jx < 0) ? ncx : 0; jx -= (jx >= ncx) ? ncx : 0;
+    for (int oy = -1; oy <= 1; ++oy) {
+      int jy = cy + oy; jy += (jy < 0) ? ncy : 0; jy -= (jy >= ncy) ? ncy : 0;
+      const int col = box * s.tnc + (jx * ncy + jy) * ncz;
+      // up to three runs: the in-range z cells, plus the wrapped cell on either side
+      for (int run = 0; run < 3; ++run) {
+        int c0, c1;
+        if (run == 0) { c0 = col + zlo; c1 = col + zhi; }
+        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; }
+        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; }
+        const int jbeg = s.cell_start[c0], jend = s.cell_start[c1 + 1];
+        for (int j = jbeg; j < jend; ++j) {
+          const double4 pj = s.pos[j];
+          unsigned kx, ky, kz;
+          const double dx = min_image(__dsub_rn(pj.x, pi.x), s.L[0], s.hL[0], kx);
+          const double dy = min_image(__dsub_rn(pj.y, pi.y), s.L[1], s.hL[1], ky);
+          const double dz = min_image(__dsub_rn(pj.z, pi.z), s.L[2], s.hL[2], kz);
+          const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          if (r2 < s.rl2 && j != i) {
+            if (n < s.cap) row[(size_t)n * 32] = (unsigned)j | ((kx | (ky << 2) | (kz << 4)) << kIdxBits);
+            ++n;
+          }
+        }
+      }
+    }
+  }
+  if (n > s.cap) { atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW); }
+  atomicMax(&s.st->max_neighbors, n);
+  s.ncount[i] = min(n, s.cap);
+}
+
+// ---- K10: close the chain ---------------------------------------------------------------------------
+__global__ void k_rebuild_end(const __grid_constant__ DevSys s) {
+  DevState *st = s.st;
+  if (st->do_rebuild) st->rebuilds += 1;
+  st->maxd2_bits = 0ull;
+  st->force_rebuild = 0;
+}
+
+int launch_rebuild_chain(md_system *sys) {
+  const DevSys &d = sys->d;
+  cudaStream_t st = sys->stream;
+  const int N = d.N, tb = 256, gN = (N + tb - 1) / tb;
+  const unsigned long long thr_bits = (unsigned long long)__builtin_bit_cast(long long, d.thr2);
+  const int nscan = (d.ncell + 1 + kScanTile - 1) / kScanTile;
+  {
+    ProfScope p(sys, MD_K_BIN);
+    int g0 = (d.ncell + 1 + tb - 1) / tb; if (g0 > 1184) g0 = 1184;
+    k_rebuild_begin<<<g0, tb, 0, st>>>(d, thr_bits);
+    k_bin<<<gN, tb, 0, st>>>(d);
+  }
+  {
+    ProfScope p(sys, MD_K_SCAN);
+    k_scan_local<<<nscan, kScanThreads, 0, st>>>(d);
+    k_scan_blocks<<<1, kScanThreads, 0, st>>>(d, nscan);
+    k_scan_add<<<nscan, kScanThreads, 0, st>>>(d);
+  }
+  {
+    ProfScope p(sys, MD_K_SORT);
+    k_scatter<<<gN, tb, 0, st>>>(d);
+    k_cell_sort<<<(d.ncell + 127) / 128, 128, 0, st>>>(d);
+  }
+  {
+    ProfScope p(sys, MD_K_REORDER);
+    k_reorder<<<gN, tb, 0, st>>>(d);
+    k_copyback<<<gN, tb, 0, st>>>(d);
+  }
+  {
+    ProfScope p(sys, MD_K_LIST);
+    k_build_list<<<d.nb * blocks_per_box(d.npb, kForceBlock), kForceBlock, 0, st>>>(d);
+    k_rebuild_end<<<1, 1, 0, st>>>(d);
+  }
+  return (int)cudaGetLastError();
+}
+
+}  // namespace md

@@ -1,0 +1,211 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the same seeded
+inputs.  Tolerances are BASELINE.json's north_star: neighbour pair sets bit-exact; |dF| <= 1e-9 eV/A per
+component; total energy relative error <= 1e-12; positions after 100 steps within 1e-8 A."""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+F_TOL, E_REL, X_TOL = 1e-9, 1e-12, 1e-8
+
+
+@pytest.fixture(scope="module")
+def md():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import paper_1212_6332_b200 as m
+    m.lib()
+    return m
+
+
+def oracle_of(w, **kw):
+    from oracle import Oracle
+    return Oracle(w, **kw)
+
+
+CASES = {
+    "cfg0": lambda: workloads.config(0),                                   # 864 Cu, 4^3 cells, 7 tiles of 128 + ragged tail
+    "cfg0_perm": lambda: workloads.permuted(workloads.config(0), 99)[0],   # caller order != any lattice order
+    "cfg1_small": lambda: workloads.config(1, scale=10),                   # 2000 Fe, tables, 5^3 cells
+    "cfg2_small": lambda: workloads.config(2, scale=7),                    # 7 boxes x 500: 3^3 cells each, images everywhere
+    "cfg3a_small": lambda: workloads.config("3a", scale=12),               # 6912 Cu
+    "cfg3b_small": lambda: workloads.config("3b", scale=12),               # 6.5 A cut-off, ~134 list entries
+    "cfg4_small": lambda: workloads.config(4, scale=12),                   # W tables + PKA
+    "noncubic": lambda: _noncubic(),
+}
+
+
+def _noncubic():
+    w = workloads.config(0, scale=5)
+    s = np.array([1.0, 1.13, 1.31])
+    w.box = w.box * s
+    w.positions = w.positions * s + np.array([40.0, -33.0, 1000.0])        # far outside the box: the build wraps
+    return w
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_neighbor_pair_sets_bit_exact(md, case):
+    w = CASES[case]()
+    o = oracle_of(w)
+    o.build_neighbors()
+    oc, ol = o.neighbors(stride=192)
+    g = md.MDSystem(w)
+    g.build_neighbors()
+    gc, gl = g.neighbors(stride=192)
+    assert np.array_equal(gc, oc)
+    assert np.array_equal(gl, ol)
+    st = g.stats()
+    assert st["max_neighbors"] == oc.max() and st["error_flags"] == 0 and st["rebuilds"] == 1
+    # device-pointer outputs give the same thing
+    dc, dl = g.neighbors(stride=192, device_out=True)
+    assert np.array_equal(dc.cpu().numpy(), oc) and np.array_equal(dl.cpu().numpy(), ol)
+    # wrapped positions agree bit for bit with the oracle's wrap
+    assert np.array_equal(g.positions(), o.positions())
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_density_force_energy_virial(md, case):
+    w = CASES[case]()
+    o = oracle_of(w)
+    of, oe, ow = o.compute_forces()
+    orho, ofp = o.densities()
+    g = md.MDSystem(w)
+    gf, ge, gw = g.compute_forces()
+    grho, gfp = g.densities()
+    assert np.abs(grho - orho).max() <= 1e-12 * np.abs(orho).max()
+    assert np.abs(gfp - ofp).max() <= 1e-12 * np.abs(ofp).max()
+    assert np.abs(gf - of).max() <= F_TOL
+    assert np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    oep, oek = o.energies()
+    gep, gek = g.energies()
+    assert np.abs(gep - oep).max() <= E_REL * np.abs(oep).max()
+    assert np.abs(gek - oek).max() <= E_REL * max(np.abs(oek).max(), 1e-300)
+    assert np.abs(gw - ow).max() <= 1e-11 * np.abs(ow).max()
+    # device outputs
+    df, de, dw = g.compute_forces(device_out=True)
+    assert np.array_equal(df.cpu().numpy(), gf) and np.array_equal(de.cpu().numpy(), ge) and np.array_equal(dw.cpu().numpy(), gw)
+
+
+@pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 100), ("cfg1_small", 100), ("cfg2_small", 100),
+                                         ("cfg3b_small", 40), ("cfg4_small", 100)])
+def test_trajectory(md, case, nsteps):
+    w = CASES[case]()
+    o = oracle_of(w)
+    g = md.MDSystem(w)
+    e0 = sum(x.sum() for x in g.energies())
+    o.step(nsteps, w.dt)
+    g.step(nsteps, w.dt)
+    ox, gx = o.positions(), g.positions()
+    d = gx - ox
+    d -= np.round(d / w.box) * w.box            # the two sides may have wrapped at different steps
+    assert np.abs(d).max() <= X_TOL
+    assert np.abs(g.velocities() - o.velocities()).max() <= 1e-9
+    so, sg = o.stats(), g.stats()
+    assert sg["steps"] == nsteps and sg["error_flags"] == 0
+    assert abs(sg["rebuilds"] - so["rebuilds"]) <= 1
+    oep, oek = o.energies()
+    gep, gek = g.energies()
+    assert abs((gep.sum() + gek.sum()) - (oep.sum() + oek.sum())) <= 1e-10 * abs(oep.sum())
+    if case.startswith("cfg0"):
+        assert abs(gep.sum() + gek.sum() - e0) / w.n_atoms < 5e-6          # NVE on the device too
+    # the list the device holds now is the oracle's list for the device's current positions
+    g.build_neighbors()
+    o2 = oracle_of(w, positions=g.positions())
+    o2.build_neighbors()
+    assert np.array_equal(g.neighbors(192)[1], o2.neighbors(192)[1])
+
+
+def test_step_with_observables_matches_plain_step(md):
+    w = CASES["cfg0"]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    b.set_option(md.MD_OPT_STEP_OBSERVABLES, 1)
+    a.step(25, 1.0)
+    b.step(25, 1.0)
+    # same arithmetic up to the contraction choices the compiler makes in the two kernel variants
+    assert np.abs(a.positions() - b.positions()).max() < 1e-11 and np.abs(a.velocities() - b.velocities()).max() < 1e-12
+
+
+def test_run_to_run_determinism(md):
+    w = CASES["cfg2_small"]()
+    res = []
+    for _ in range(2):
+        g = md.MDSystem(w)
+        g.step(30, 1.0)
+        res.append((g.positions(), g.compute_forces()[0], g.energies()[0]))
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1]) and np.array_equal(res[0][2], res[1][2])
+
+
+def test_set_get_roundtrip_and_device_inputs(md):
+    import torch
+    w = CASES["cfg0_perm"]()
+    g = md.MDSystem(w)
+    assert np.array_equal(g.velocities(), w.velocities)
+    g.build_neighbors()
+    x = g.positions()
+    v2 = np.random.default_rng(0).standard_normal(x.shape) * 0.01
+    g.set_velocities(torch.from_numpy(v2).cuda())
+    assert np.array_equal(g.velocities(), v2)
+    f0 = g.compute_forces()[0]
+    g.set_positions(x + 0.01)                    # rigid shift below skin/2: list kept, forces unchanged
+    f1 = g.compute_forces()[0]
+    assert g.stats()["rebuilds"] == 1 and np.abs(f1 - f0).max() < 1e-10
+    g.set_positions(torch.from_numpy(x + w.box * np.array([1.0, -2.0, 3.0])).cuda())   # other periodic image
+    assert np.abs(g.compute_forces()[0] - f0).max() < 1e-10 and g.stats()["rebuilds"] == 1
+    g.set_positions(x + np.array([0.2, 0.0, 0.0]))   # beyond skin/2: must rebuild
+    f2 = g.compute_forces()[0]
+    assert g.stats()["rebuilds"] == 2 and np.abs(f2 - f0).max() < 1e-10
+    # a system created from device tensors equals one created from host arrays
+    gd = md.MDSystem(w, positions=torch.from_numpy(w.positions).cuda(), velocities=torch.from_numpy(w.velocities).cuda(),
+                     types=torch.from_numpy(w.types).cuda())
+    assert np.array_equal(gd.compute_forces()[0], md.MDSystem(w).compute_forces()[0])
+
+
+def test_error_codes(md):
+    w = workloads.config(0, scale=4)             # L = 14.46 < 3 * 5.2
+    with pytest.raises(md.MDError) as ei:
+        md.MDSystem(w)
+    assert ei.value.code == md.MD_EBOX
+    w = workloads.config(0, scale=5)
+    g = md.MDSystem(w, max_neighbors=20)
+    g.build_neighbors()
+    with pytest.raises(md.MDError) as ei:
+        g.neighbors()
+    assert ei.value.code == md.MD_EOVERFLOW and g.stats()["error_flags"] & md.MD_FLAG_OVERFLOW
+    w.positions[1] = w.positions[0]
+    g = md.MDSystem(w)
+    with pytest.raises(md.MDError) as ei:
+        g.compute_forces()
+    assert ei.value.code == md.MD_ENONFINITE
+    w = workloads.config(0, scale=5)
+    w.positions[7, 1] = np.nan
+    g = md.MDSystem(w)
+    with pytest.raises(md.MDError) as ei:
+        g.compute_forces()
+    assert ei.value.code == md.MD_ENONFINITE
+    w = workloads.config(0, scale=5)
+    with pytest.raises(md.MDError) as ei:
+        md.MDSystem(w, types=np.full(w.n_atoms, 2, np.int32))
+    assert ei.value.code == md.MD_EINVAL
+    g = md.MDSystem(w)
+    with pytest.raises(md.MDError) as ei:
+        g.neighbors()
+    assert ei.value.code == md.MD_ESTATE
+
+
+def test_sparse_and_tiny_systems(md):
+    """degenerate inputs: atoms with no neighbour at all, a box holding two atoms, a one-atom box batch."""
+    base = dict(box=np.full(3, 40.0), velocities=None, cutoff=4.9, skin=0.3, n_boxes=1, pot_kind=0,
+                mass=np.array([63.546]), tbsma=workloads.cu_tbsma_params(4.9))
+    pos = np.array([[1.0, 1.0, 1.0], [20.0, 20.0, 20.0]])
+    g = md.MDSystem(positions=pos, types=np.zeros(2, np.int32), **base)
+    f, e, wv = g.compute_forces()
+    assert np.all(f == 0) and np.all(e == 0) and np.all(wv == 0) and np.all(g.neighbors()[0] == 0)
+    pos = np.array([[39.5, 0.2, 20.0], [1.5, 39.9, 20.0]])                # neighbours only through the periodic images
+    g = md.MDSystem(positions=pos, types=np.zeros(2, np.int32), **base)
+    o = oracle_of(None, positions=pos, types=np.zeros(2, np.int32), velocities=np.zeros((2, 3)), **{k: v for k, v in base.items() if k != "velocities"})
+    assert np.abs(g.compute_forces()[0] - o.compute_forces()[0]).max() < 1e-12 and np.abs(g.compute_forces()[0]).max() > 0.1
+    pos = np.tile(np.array([[3.0, 4.0, 5.0]]), (6, 1))                     # 6 boxes x 1 atom: never a neighbour
+    g = md.MDSystem(positions=pos, types=np.zeros(6, np.int32), **{**base, "n_boxes": 6})
+    assert np.all(g.compute_forces()[0] == 0) and g.energies()[0].shape == (6,)
