@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py — FP64 atom-steps/s of the EAM / TB-SMA MD hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3a|3b|0|1|2|4] [--impl reference]
+
+A "step" is one velocity-Verlet time step of the whole hot path (kick+drift+displacement check, the
+displacement-triggered neighbour rebuild when it fires, density pass, force pass, second half-kick) over
+one synthetic system; K steps are one `md_step(K, dt)` call through the C ABI.  The default workload is
+BASELINE.json configs[3] at cut-off 4.9 A (Cu fcc 64^3 = 1,048,576 atoms, TB-SMA): the case north_star
+quotes the roofline fraction on.  Prints ONE JSON line (rank 0).
+
+Keys beyond the base contract:
+  roofline      the dominant kernel (force pass): algorithmic FP64-pipe instructions per launch / its mean
+                CUDA-event duration, against the FP64 issue rate measured by md_fp64_dfma_rate in this run
+                ("bound": "alu"); `hbm` inside it gives the same kernel's algorithmic bytes / duration
+                against MEASURED_PEAKS.json's copy bandwidth.  Per-unit figures: DESIGN.md section 7.
+  kernels       device time per kernel class over a separately profiled run of the same K steps.
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+  e2e           the same metric with HOST buffers: every step copies positions and velocities host->device
+                (pinned), runs md_step(1), and copies them back.
+Multi-GPU (--gpus N under torchrun): replicas only — one independent system per GPU, no collective on the
+data path; value = all ranks' atom-steps / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import workloads
+
+METRIC = "FP64 atom-steps/s"
+UNIT = "atom-steps/s"
+
+# Perfect-lattice pair counts (SURVEY.md section 8 geometry table): in-cutoff neighbours per atom.
+IN_CUTOFF = {"0": 42, "1": 58, "2": 42, "3a": 42, "3": 42, "3b": 86, "4": 58}
+# bounded oracle sample: unit cells per edge (boxes for config 2) of the reduced system of the same kind
+SAMPLE_SCALE = {"0": 6, "1": 24, "2": 64, "3a": 24, "3": 24, "3b": 20, "4": 24}
+
+# Algorithmic FP64-pipe instruction counts: per LISTED pair and pass the distance test;
+# per IN-CUTOFF pair the potential terms.  TB-SMA: sqrt + 1 (density) or 2 (force) exp + quintic switch;
+# tables: sqrt + 1 (density) or 2 (force) cubic-Hermite evaluations with derivative.
+SLOTS = {
+    0: dict(dist=9, dens=45, force=95),     # MD_POT_TBSMA
+    1: dict(dist=9, dens=25, force=60),     # MD_POT_EAM_TABLE
+}
+
+
+def algorithmic(kind: int, n_atoms: int, list_entries: float, in_cutoff: float) -> dict:
+    """Algorithmic work of ONE force-pass launch and ONE density-pass launch."""
+    m = list_entries / n_atoms
+    s = SLOTS[kind]
+    return dict(
+        force_slots=n_atoms * (m * s["dist"] + in_cutoff * s["force"]),
+        dens_slots=n_atoms * (m * s["dist"] + in_cutoff * s["dens"]),
+        force_bytes=n_atoms * (4 * m + 4 + 32 + 24 + 24 + 24),   # ids, count, own pos+F', force out, vel in/out (fused kick)
+        dens_bytes=n_atoms * (4 * m + 4 + 32 + 32 + 8),          # ids, count, own pos, pos+F' out, embedding energy out
+    )
+
+
+class ClockSampler(threading.Thread):
+    """SM clock and throttle reasons of one GPU, sampled with NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.01):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.max_mhz, self.ok = period, [], set(), None, False
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+                 "hw_power_brake": getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80)}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join()
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def measured_peaks() -> tuple[float, str]:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:  # noqa: BLE001
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# --------------------------------------------------------------------------------------------------------
+# the CPU oracle: cpu_baseline leg and --impl reference arm
+# --------------------------------------------------------------------------------------------------------
+def oracle_sample(workload: str):
+    from oracle import Oracle, set_threads
+    cores = set_threads(0)
+    w = workloads.config(workload, scale=SAMPLE_SCALE[workload])
+    return Oracle(w), w, cores
+
+
+def time_oracle(workload: str, budget_s: float) -> dict:
+    """atom-steps/s of the oracle on a bounded sample; about `budget_s` seconds of wall time."""
+    o, w, cores = oracle_sample(workload)
+    t0 = time.perf_counter()
+    o.step(1, w.dt)                       # builds the list and evaluates the initial forces: untimed warm-up
+    t_first = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.step(2, w.dt)
+    per = (time.perf_counter() - t0) / 2
+    n = int(max(3, min(w.steps, budget_s / max(per, 1e-6))))
+    r0 = o.stats()["rebuilds"]
+    t0 = time.perf_counter()
+    o.step(n, w.dt)
+    t = time.perf_counter() - t0
+    return {"value": w.n_atoms * n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{w.name} reduced to {w.n_atoms} atoms ({SAMPLE_SCALE[workload]} per edge), {n} steps of dt={w.dt} fs "
+                      f"incl. {o.stats()['rebuilds'] - r0} rebuilds, OpenMP over atoms, full (directed) lists; "
+                      f"first step (list build + 2 force evaluations) {t_first:.2f} s untimed",
+            "ms_per_step": 1e3 * t / n}
+
+
+def reference_arm(args, rank: int):
+    if rank != 0:
+        return
+    o, w, cores = oracle_sample(args.workload)
+    o.step(max(args.warmup, 1), w.dt)
+    t0 = time.perf_counter()
+    o.step(args.steps, w.dt)
+    t = time.perf_counter() - t0
+    value = w.n_atoms * args.steps / t
+    sample = (f"{w.name} reduced to {w.n_atoms} atoms ({SAMPLE_SCALE[args.workload]} per edge); every step is one "
+              f"oracle_step of that sample on the host cores")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": full_name(args.workload), "sample_atoms": w.n_atoms},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+FULL_NAMES = {"0": "cfg0_cu_fcc6_tbsma", "1": "cfg1_fe_bcc32_eam", "2": "cfg2_cu_fcc5_x2048_tbsma", "3": "cfg3a_cu_fcc64_rc4.9",
+              "3a": "cfg3a_cu_fcc64_rc4.9", "3b": "cfg3b_cu_fcc64_rc6.5", "4": "cfg4_w_bcc128_eam_pka"}
+
+
+def full_name(k: str) -> str:
+    return FULL_NAMES[k]
+
+
+# --------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------------------------
+def cuda_arm(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    import paper_1212_6332_b200 as md
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    md.lib()                                         # fails loudly if libmd_b200.so cannot be built / loaded
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = workloads.config(args.workload, scale=args.scale, replica=rank)
+    K, W = args.steps, args.warmup
+    g = md.MDSystem(w)
+    stream = torch.cuda.current_stream()
+
+    # ---- device-resident run: W warm-up steps, then exactly K timed steps ------------------------------
+    g.step(W, w.dt)
+    st0 = g.stats()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    g.step(K, w.dt)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    st1 = g.stats()
+    if st1["error_flags"]:
+        raise SystemExit(f"device error flags {st1['error_flags']}")
+    launches = st1["kernel_launches"] - st0["kernel_launches"]
+    rebuilds = st1["rebuilds"] - st0["rebuilds"]
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * w.n_atoms * K / (ms_max * 1e-3)
+
+    # ---- per-kernel device time over the same K steps, events around every launch (separate run) --------
+    g.set_option(md.MD_OPT_PROFILE, 1)
+    g.profile_reset()
+    g.step(K, w.dt)
+    prof = g.profile()
+    st2 = g.stats()
+    g.set_option(md.MD_OPT_PROFILE, 0)
+    tot = sum(v[1] for v in prof.values())
+    kernels = {k: {"launches": v[0], "ms": round(v[1], 4), "share": round(v[1] / tot, 4)} for k, v in prof.items() if v[0]}
+    dfma_rate, dfma_mhz = md.fp64_dfma_rate()
+    hbm_peak, hbm_src = measured_peaks()
+    alg = algorithmic(w.pot_kind, w.n_atoms, st2["list_entries"], IN_CUTOFF[args.workload])
+    f_ms = prof["force"][1] / prof["force"][0]
+    d_ms = prof["density"][1] / prof["density"][0]
+    roofline = {
+        "kernel": "k_force (force pass + fused second half-kick)", "bound": "alu",
+        "achieved": alg["force_slots"] / (f_ms * 1e-3) / 1e12, "peak": dfma_rate / 1e12, "unit": "T FP64-inst/s",
+        "frac": alg["force_slots"] / (f_ms * 1e-3) / dfma_rate, "traffic": None,
+        "peak_source": f"md_fp64_dfma_rate measured in this run at {dfma_mhz:.0f} MHz",
+        "ms_per_launch": f_ms, "algorithmic_fp64_inst_per_launch": alg["force_slots"],
+        "hbm": {"achieved": alg["force_bytes"] / (f_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": alg["force_bytes"] / (f_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
+                "algorithmic_bytes_per_launch": alg["force_bytes"]},
+        "density": {"ms_per_launch": d_ms, "achieved": alg["dens_slots"] / (d_ms * 1e-3) / 1e12,
+                    "frac": alg["dens_slots"] / (d_ms * 1e-3) / dfma_rate,
+                    "hbm_frac": alg["dens_bytes"] / (d_ms * 1e-3) / 1e9 / hbm_peak},
+    }
+
+    # ---- end to end with HOST buffers: H2D of x and v, one step, D2H of x and v, every step --------------
+    e2e = None
+    if not args.no_e2e:
+        n = w.n_atoms
+        hx = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+        hv = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+        hxn, hvn = hx.numpy(), hv.numpy()
+        g.positions(out=hxn)
+        g.velocities(out=hvn)
+        Ke = min(K, args.e2e_steps) if args.e2e_steps else K
+        for _ in range(3):
+            g.set_positions(hxn); g.set_velocities(hvn); g.step(1, w.dt); g.positions(out=hxn); g.velocities(out=hvn)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            g.set_positions(hxn)
+            g.set_velocities(hvn)
+            g.step(1, w.dt)
+            g.positions(out=hxn)
+            g.velocities(out=hvn)
+        barrier()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n * Ke / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
+               "steps": Ke, "ms_per_step": 1e3 * float(te.item()) / Ke,
+               "what": "per step: md_set_positions + md_set_velocities from pinned host arrays, md_step(1) (forces are "
+                       "re-evaluated for the new positions, then one velocity-Verlet step), md_get_positions + md_get_velocities"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = time_oracle(args.workload, args.cpu_seconds)
+
+    if rank == 0:
+        ws_mb = g.workspace_bytes / 2 ** 20
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_atoms_per_gpu": w.n_atoms, "n_boxes": w.n_boxes, "cutoff": w.cutoff, "skin": w.skin,
+                       "dt_fs": w.dt, "parallelism": "replicas only (one independent system per GPU, no collective)",
+                       "rebuilds_in_timed_region": rebuilds, "mean_list_entries": st2["list_entries"] / w.n_atoms,
+                       "l2": f"no flush: per-step working set (neighbour list {4 * st2['list_entries'] / 2 ** 20:.0f} MiB + per-atom "
+                             f"arrays, workspace {ws_mb:.0f} MiB) exceeds the 126 MB L2" if 4 * st2["list_entries"] > 126e6
+                             else "no flush: working set fits L2 (small config; steady-state MD keeps it there by design)"},
+            "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="3a", choices=sorted(IN_CUTOFF))
+    ap.add_argument("--scale", type=int, default=None, help="reduced size (unit cells per edge / boxes); default: full size")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline leg")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="cap on the end-to-end steps (0: same as --steps)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.gpus > 1 and world == 1:
+        raise SystemExit("launch with: python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N")
+    if args.impl == "reference":
+        reference_arm(args, rank)
+    else:
+        cuda_arm(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

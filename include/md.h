@@ -98,6 +98,8 @@ typedef struct {
   int error_flags;                /* MD_FLAG_* bits, sticky */
   double last_max_disp2;          /* max_i |x_i - x_ref,i|^2 at the last displacement check (Angstrom^2) */
   int neighbor_capacity;          /* list capacity per atom in use */
+  long kernel_launches;           /* CUDA kernels this system has enqueued since md_create (host-side count) */
+  long list_entries;              /* sum over atoms of the list lengths of the last build (directed pairs) */
 } md_stats;
 
 /* Bytes of device workspace md_create needs for this description (pointers in *d are not read). */

@@ -320,7 +320,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->stream = (cudaStream_t)d->stream;
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
-  s->opt_step_obs = s->opt_profile = false; s->opt_force_variant = 0; s->steps = 0;
+  s->opt_step_obs = s->opt_profile = false; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
   o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
@@ -364,7 +364,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     tdev = o.cell_id;
   }
   if (e == cudaSuccess) {
-    k_init_atoms<<<grid_for(o.N), 256, 0, st>>>(o, xdev, tdev);
+    ++s->launches, k_init_atoms<<<grid_for(o.N), 256, 0, st>>>(o, xdev, tdev);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) {
@@ -373,7 +373,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
       e = cudaMemcpyAsync(s->stage, vdev, 3 * N * sizeof(double), cudaMemcpyHostToDevice, st);   // stream order: after k_init_atoms
       vdev = (const double *)s->stage;
     }
-    if (e == cudaSuccess) { k_set_vec<<<grid_for(o.N), 256, 0, st>>>(o, o.vel, vdev); e = cudaGetLastError(); }
+    if (e == cudaSuccess) { ++s->launches, k_set_vec<<<grid_for(o.N), 256, 0, st>>>(o, o.vel, vdev); e = cudaGetLastError(); }
   }
   if (e == cudaSuccess) e = cudaMemsetAsync(o.frc, 0, 3 * N * sizeof(double), st);
   int flags = 0;
@@ -419,17 +419,17 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
   bool any_host = false, h;
   double *scratch = (double *)s->stage;
   if (forces) {
-    if (on_device(forces)) k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, forces);
+    if (on_device(forces)) ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, forces);
     else {
-      k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, scratch);
+      ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.frc, scratch);
       if ((rc = deliver(s, forces, scratch, 3 * (size_t)o.N * sizeof(double), &h)) != MD_OK) return rc;
       any_host = true;
     }
   }
   if (e_atom) {
-    if (on_device(e_atom)) k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, e_atom);
+    if (on_device(e_atom)) ++s->launches, k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, e_atom);
     else {
-      k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, scratch);   // stream order: after the copy above
+      ++s->launches, k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, scratch);   // stream order: after the copy above
       if ((rc = deliver(s, e_atom, scratch, (size_t)o.N * sizeof(double), &h)) != MD_OK) return rc;
       any_host = true;
     }
@@ -459,8 +459,8 @@ int md_step(md_system *s, int n, double dt) {
 int md_get_positions(md_system *s, double *x) {
   if (!s || !x) return MD_EINVAL;
   const DevSys &o = s->d;
-  if (on_device(x)) { k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, x); return check_cuda(cudaGetLastError()); }
-  k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, (double *)s->stage);
+  if (on_device(x)) { ++s->launches, k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, x); return check_cuda(cudaGetLastError()); }
+  ++s->launches, k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, (double *)s->stage);
   int rc = deliver(s, x, s->stage, 3 * (size_t)o.N * sizeof(double), nullptr);
   return rc != MD_OK ? rc : sync_and_flags(s);
 }
@@ -468,8 +468,8 @@ int md_get_positions(md_system *s, double *x) {
 int md_get_velocities(md_system *s, double *v) {
   if (!s || !v) return MD_EINVAL;
   const DevSys &o = s->d;
-  if (on_device(v)) { k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, v); return check_cuda(cudaGetLastError()); }
-  k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, (double *)s->stage);
+  if (on_device(v)) { ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, v); return check_cuda(cudaGetLastError()); }
+  ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, (double *)s->stage);
   int rc = deliver(s, v, s->stage, 3 * (size_t)o.N * sizeof(double), nullptr);
   return rc != MD_OK ? rc : sync_and_flags(s);
 }
@@ -482,7 +482,7 @@ int md_set_positions(md_system *s, const double *x) {
     if (cudaMemcpyAsync(s->stage, x, 3 * (size_t)o.N * sizeof(double), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
     src = (const double *)s->stage;
   }
-  k_set_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, src, s->have_list ? 1 : 0);
+  ++s->launches, k_set_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, src, s->have_list ? 1 : 0);
   s->forces_valid = false; s->observables_valid = false;
   if (src != x && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;   // the host buffer may be reused
   return check_cuda(cudaGetLastError());
@@ -496,7 +496,7 @@ int md_set_velocities(md_system *s, const double *v) {
     if (cudaMemcpyAsync(s->stage, v, 3 * (size_t)o.N * sizeof(double), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
     src = (const double *)s->stage;
   }
-  k_set_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, src);
+  ++s->launches, k_set_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, src);
   if (src != v && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   return check_cuda(cudaGetLastError());
 }
@@ -509,9 +509,9 @@ int md_get_neighbors(md_system *s, int *count, int *list, int stride) {
   if (dev != on_device(count)) return MD_EINVAL;       // both on the same side
   int *flag = o.scan_block;                            // free outside the rebuild chain
   if (cudaMemsetAsync(flag, 0, sizeof(int), s->stream) != cudaSuccess) return MD_ECUDA;
-  k_invert_orig<<<grid_for(o.N), 256, 0, s->stream>>>(o);
+  ++s->launches, k_invert_orig<<<grid_for(o.N), 256, 0, s->stream>>>(o);
   if (dev) {
-    k_export_neighbors<<<grid_for(o.N, 128), 128, 0, s->stream>>>(o, 0, o.N, count, list, stride, flag);
+    ++s->launches, k_export_neighbors<<<grid_for(o.N, 128), 128, 0, s->stream>>>(o, 0, o.N, count, list, stride, flag);
   } else {
     // chunks of caller atoms that fit the staging area: [chunk] counts followed by [chunk][stride] rows
     const size_t per_atom = ((size_t)stride + 1) * sizeof(int);
@@ -520,7 +520,7 @@ int md_get_neighbors(md_system *s, int *count, int *list, int stride) {
     int *dcount = (int *)s->stage, *dlist = dcount + chunk;
     for (int first = 0; first < o.N; first += chunk) {
       const int na = o.N - first < chunk ? o.N - first : chunk;
-      k_export_neighbors<<<grid_for(na, 128), 128, 0, s->stream>>>(o, first, na, dcount, dlist, stride, flag);
+      ++s->launches, k_export_neighbors<<<grid_for(na, 128), 128, 0, s->stream>>>(o, first, na, dcount, dlist, stride, flag);
       if (cudaMemcpyAsync(count + first, dcount, (size_t)na * sizeof(int), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
           cudaMemcpyAsync(list + (size_t)first * stride, dlist, (size_t)na * stride * sizeof(int), cudaMemcpyDeviceToHost,
                           s->stream) != cudaSuccess)
@@ -542,17 +542,17 @@ int md_get_densities(md_system *s, double *rho, double *fprime) {
   bool any_host = false;
   double *scratch = (double *)s->stage;
   if (rho) {
-    if (on_device(rho)) k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, rho);
+    if (on_device(rho)) ++s->launches, k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, rho);
     else {
-      k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, scratch);
+      ++s->launches, k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.rho, scratch);
       if ((rc = deliver(s, rho, scratch, (size_t)o.N * sizeof(double), nullptr)) != MD_OK) return rc;
       any_host = true;
     }
   }
   if (fprime) {
-    if (on_device(fprime)) k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, fprime);
+    if (on_device(fprime)) ++s->launches, k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, fprime);
     else {
-      k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, scratch);
+      ++s->launches, k_get_fprime<<<grid_for(o.N), 256, 0, s->stream>>>(o, scratch);
       if ((rc = deliver(s, fprime, scratch, (size_t)o.N * sizeof(double), nullptr)) != MD_OK) return rc;
       any_host = true;
     }
@@ -583,7 +583,7 @@ int md_get_stats(md_system *s, md_stats *out) {
   if (cudaMemcpyAsync(&st, s->d.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
   if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   out->steps = s->steps; out->rebuilds = (long)st.rebuilds; out->max_neighbors = st.max_neighbors;
-  out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap;
+  out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap; out->kernel_launches = s->launches; out->list_entries = (long)st.list_entries;
   return MD_OK;
 }
 

@@ -227,8 +227,8 @@ __global__ void __launch_bounds__(256) k_reduce_boxes(const __grid_constant__ De
 
 template <int KIND>
 static void launch_density_k(md_system *sys, int grid) {
-  if (sys->d.nt > 1) k_density<KIND, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-  else k_density<KIND, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  if (sys->d.nt > 1) ++sys->launches, k_density<KIND, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  else ++sys->launches, k_density<KIND, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
 }
 
 int launch_density(md_system *sys) {
@@ -241,8 +241,8 @@ int launch_density(md_system *sys) {
 
 template <int KIND, bool MULTI>
 static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams &kp) {
-  if (obs) k_force<KIND, MULTI, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, kp);
-  else k_force<KIND, MULTI, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, kp);
+  if (obs) ++sys->launches, k_force<KIND, MULTI, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, kp);
+  else ++sys->launches, k_force<KIND, MULTI, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, kp);
 }
 
 int launch_force(md_system *sys, bool observables, double half_dt) {
@@ -262,7 +262,7 @@ int launch_force(md_system *sys, bool observables, double half_dt) {
   }
   if (observables) {
     ProfScope p(sys, MD_K_REDUCE);
-    k_reduce_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, blocks_per_box(sys->d.npb, kForceBlock));
+    ++sys->launches, k_reduce_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, blocks_per_box(sys->d.npb, kForceBlock));
   }
   return (int)cudaGetLastError();
 }

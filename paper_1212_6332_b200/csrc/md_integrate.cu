@@ -46,7 +46,7 @@ int launch_kick_drift(md_system *sys, double dt) {
   DtParams dp;
   dp.dt = dt;
   for (int t = 0; t < MD_MAX_TYPES; ++t) dp.h[t] = (t < sys->d.nt) ? 0.5 * dt / sys->mass_ev[t] : 0.0;
-  k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, dp);
+  ++sys->launches, k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, dp);
   return (int)cudaGetLastError();
 }
 
@@ -95,8 +95,8 @@ int launch_ekin(md_system *sys) {
   MassParams mp;
   for (int t = 0; t < MD_MAX_TYPES; ++t) mp.m[t] = (t < sys->d.nt) ? sys->mass_ev[t] : 0.0;
   const int bpb = blocks_per_box(sys->d.npb, kForceBlock);
-  k_ekin_partial<<<sys->d.nb * bpb, kForceBlock, 0, sys->stream>>>(sys->d, mp);
-  k_ekin_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, bpb);
+  ++sys->launches, k_ekin_partial<<<sys->d.nb * bpb, kForceBlock, 0, sys->stream>>>(sys->d, mp);
+  ++sys->launches, k_ekin_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, bpb);
   return (int)cudaGetLastError();
 }
 

@@ -25,6 +25,7 @@ struct DevState {
   int error_flags;                 // MD_FLAG_* (sticky)
   int max_neighbors;               // of the last build
   unsigned long long rebuilds;
+  unsigned long long list_entries; // sum of list lengths of the last build
 };
 
 struct TbsmaParams {               // per type pair, pre-combined on the host
@@ -83,7 +84,7 @@ struct md_system {
   bool have_list, forces_valid, observables_valid;
   bool opt_step_obs, opt_profile;
   int opt_force_variant;
-  long steps;
+  long steps, launches;
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
   int n_force_blocks;
   md::ProfClass prof[MD_K_COUNT];

@@ -30,7 +30,7 @@ __global__ void k_rebuild_begin(const __grid_constant__ DevSys s, unsigned long 
   if (gid == 0) {
     s.st->do_rebuild = go ? 1 : 0;
     s.st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
-    if (go) s.st->max_neighbors = 0;
+    if (go) { s.st->max_neighbors = 0; s.st->list_entries = 0ull; }
   }
 }
 
@@ -223,8 +223,14 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     }
   }
   if (n > s.cap) { atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW); }
-  atomicMax(&s.st->max_neighbors, n);
   s.ncount[i] = min(n, s.cap);
+  // statistics: one atomic per warp
+  const unsigned act = __activemask();
+  const int wsum = __reduce_add_sync(act, min(n, s.cap)), wmax = __reduce_max_sync(act, n);
+  if ((threadIdx.x & 31) == __ffs(act) - 1) {
+    atomicAdd(&s.st->list_entries, (unsigned long long)wsum);
+    atomicMax(&s.st->max_neighbors, wmax);
+  }
 }
 
 // ---- K10: close the chain ---------------------------------------------------------------------------
@@ -244,29 +250,29 @@ int launch_rebuild_chain(md_system *sys) {
   {
     ProfScope p(sys, MD_K_BIN);
     int g0 = (d.ncell + 1 + tb - 1) / tb; if (g0 > 1184) g0 = 1184;
-    k_rebuild_begin<<<g0, tb, 0, st>>>(d, thr_bits);
-    k_bin<<<gN, tb, 0, st>>>(d);
+    ++sys->launches, k_rebuild_begin<<<g0, tb, 0, st>>>(d, thr_bits);
+    ++sys->launches, k_bin<<<gN, tb, 0, st>>>(d);
   }
   {
     ProfScope p(sys, MD_K_SCAN);
-    k_scan_local<<<nscan, kScanThreads, 0, st>>>(d);
-    k_scan_blocks<<<1, kScanThreads, 0, st>>>(d, nscan);
-    k_scan_add<<<nscan, kScanThreads, 0, st>>>(d);
+    ++sys->launches, k_scan_local<<<nscan, kScanThreads, 0, st>>>(d);
+    ++sys->launches, k_scan_blocks<<<1, kScanThreads, 0, st>>>(d, nscan);
+    ++sys->launches, k_scan_add<<<nscan, kScanThreads, 0, st>>>(d);
   }
   {
     ProfScope p(sys, MD_K_SORT);
-    k_scatter<<<gN, tb, 0, st>>>(d);
-    k_cell_sort<<<(d.ncell + 127) / 128, 128, 0, st>>>(d);
+    ++sys->launches, k_scatter<<<gN, tb, 0, st>>>(d);
+    ++sys->launches, k_cell_sort<<<(d.ncell + 127) / 128, 128, 0, st>>>(d);
   }
   {
     ProfScope p(sys, MD_K_REORDER);
-    k_reorder<<<gN, tb, 0, st>>>(d);
-    k_copyback<<<gN, tb, 0, st>>>(d);
+    ++sys->launches, k_reorder<<<gN, tb, 0, st>>>(d);
+    ++sys->launches, k_copyback<<<gN, tb, 0, st>>>(d);
   }
   {
     ProfScope p(sys, MD_K_LIST);
-    k_build_list<<<d.nb * blocks_per_box(d.npb, kForceBlock), kForceBlock, 0, st>>>(d);
-    k_rebuild_end<<<1, 1, 0, st>>>(d);
+    ++sys->launches, k_build_list<<<d.nb * blocks_per_box(d.npb, kForceBlock), kForceBlock, 0, st>>>(d);
+    ++sys->launches, k_rebuild_end<<<1, 1, 0, st>>>(d);
   }
   return (int)cudaGetLastError();
 }

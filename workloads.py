@@ -188,11 +188,19 @@ def bcc_eam(ncell: int, a: float, re: float, cutoff: float, element: str, skin: 
 # --------------------------------------------------------------------------------------
 # BASELINE.json configs
 # --------------------------------------------------------------------------------------
-def config(k: int | str, scale: int | None = None) -> Workload:
+def config(k: int | str, scale: int | None = None, replica: int = 0) -> Workload:
     """BASELINE.json `configs[k]`; k = '3a' / '3b' select the two cut-offs of configs[3].
     `scale` overrides the number of unit cells per edge (boxes for config 2) for reduced
-    parity-test sizes; None gives the full size."""
+    parity-test sizes; None gives the full size.  `replica` > 0 draws an independent copy of
+    the same system (seed + 100003 * replica): bench.py gives one replica to every GPU."""
     k = str(k)
+    if replica:
+        global BASE_SEED
+        saved, BASE_SEED = BASE_SEED, BASE_SEED + 100003 * int(replica)
+        try:
+            return config(k, scale)
+        finally:
+            BASE_SEED = saved
     if k == "0":
         return cu_fcc(scale or 6, 4.9, seed=BASE_SEED + 0, steps=100, name="cfg0_cu_fcc6_tbsma")
     if k == "1":
