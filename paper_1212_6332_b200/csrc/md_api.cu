@@ -75,6 +75,7 @@ static int geometry(const md_desc *d, Geometry &g) {
   }
   if (g.cap > g.npb - 1) g.cap = g.npb - 1;
   if (g.cap < 4) g.cap = 4;
+  if (g.cap > 0xfff0) return MD_EINVAL;               // ncount packs two 16-bit counts
   g.cap = (g.cap + 3) & ~3;
   g.tiles_per_box = (g.npb + 31) / 32;
   g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock);
@@ -103,10 +104,14 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   t.box_epot = b.take<double>(d->n_boxes); t.box_virial = b.take<double>((size_t)d->n_boxes * 6);
   t.box_ekin = b.take<double>(d->n_boxes);
   double *tabs[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  double4 *coef[3] = {nullptr, nullptr, nullptr};
   if (d->pot_kind == MD_POT_EAM_TABLE) {
     for (int k = 0; k < 4; ++k) tabs[k] = b.take<double>(nt2 * d->nr);
     for (int k = 4; k < 6; ++k) tabs[k] = b.take<double>((size_t)d->n_types * d->nrho);
+    coef[0] = b.take<double4>(nt2 * (d->nr - 1)); coef[1] = b.take<double4>(nt2 * (d->nr - 1));
+    coef[2] = b.take<double4>(2 * nt2 * (d->nr - 1));
   }
+  double *exp_tab = b.take<double>(64);
   void *stage = b.take<char>(g.stage_bytes);
   if (sys) {
     DevSys &o = sys->d;
@@ -118,6 +123,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
     o.box_ekin = t.box_ekin;
     o.tab.f_val = tabs[0]; o.tab.f_der = tabs[1]; o.tab.phi_val = tabs[2]; o.tab.phi_der = tabs[3];
     o.tab.F_val = tabs[4]; o.tab.F_der = tabs[5];
+    o.tab.f_c = coef[0]; o.tab.phi_c = coef[1]; o.tab.der_c = coef[2]; o.exp_tab = exp_tab;
     sys->stage = stage; sys->stage_bytes = g.stage_bytes;
   }
   return (b.off + 255) & ~(size_t)255;
@@ -216,12 +222,13 @@ __global__ void k_export_neighbors(const __grid_constant__ DevSys s, int first, 
   const int box = i / s.npb, local = i - box * s.npb;
   const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
   const unsigned *row = s.nbr + tile * s.cap * 32 + (local & 31);
-  const int n = s.ncount[i];
+  const int c = s.ncount[i], n_in = c & 0xffff, n = n_in + (c >> 16);
   count[a] = n;
   if (n > stride) { atomicOr(overflow, 1); return; }
   int *out = list + (size_t)a * stride;
   for (int k = 0; k < n; ++k) {
-    const int v = s.orig[row[(size_t)k * 32] & kIdxMask];
+    const int kk = k < n_in ? k : s.cap - 1 - (k - n_in);        // front part, then the skin part stored from the back
+    const int v = s.orig[row[(size_t)kk * 32] & kIdxMask];
     int b = k - 1;
     while (b >= 0 && out[b] > v) { out[b + 1] = out[b]; --b; }
     out[b + 1] = v;
@@ -328,21 +335,39 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   for (int a = 0; a < 3; ++a) {
     o.L[a] = d->box[a]; o.hL[a] = 0.5 * d->box[a]; o.nc[a] = g.nc[a]; o.cell_scale[a] = (double)g.nc[a] / d->box[a];
   }
-  o.rc2 = d->cutoff * d->cutoff; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
+  o.rc2 = d->cutoff * d->cutoff; o.rin2 = o.rc2; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
   o.tnc = g.tnc; o.ncell = g.ncell; o.cap = g.cap; o.tiles_per_box = g.tiles_per_box;
   s->n_force_blocks = g.n_blocks;
   for (int t = 0; t < d->n_types; ++t) s->mass_ev[t] = d->mass[t] * kAmuToEvFs2PerA2;
   const size_t N = (size_t)o.N, nt2 = (size_t)o.nt * o.nt;
   cudaStream_t st = s->stream;
   cudaError_t e = cudaMemsetAsync(o.st, 0, sizeof(DevState), st);
+  {
+    // 2^(j/64), j = 0..63, rounded from long double (64-bit mantissa): the table of exp_tab() in md_force.cu
+    double tab[64];
+    for (int j = 0; j < 64; ++j) tab[j] = (double)exp2l((long double)j / 64.0L);
+    if (e == cudaSuccess) e = cudaMemcpyAsync((void *)o.exp_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // tab is on this stack frame
+  }
   if (d->pot_kind == MD_POT_TBSMA) {
+    bool fold = true;
     for (size_t k = 0; k < nt2; ++k) {
       if (!(d->r0[k] > 0.0)) { delete s; return MD_EINVAL; }
-      o.tb.A2[k] = 2.0 * d->A[k]; o.tb.xi2[k] = d->xi[k] * d->xi[k];
-      o.tb.p[k] = d->p[k]; o.tb.p_r0[k] = d->p[k] / d->r0[k];
-      o.tb.q2[k] = 2.0 * d->q[k]; o.tb.q2_r0[k] = 2.0 * d->q[k] / d->r0[k];
+      if (!(d->A[k] > 0.0) || !(d->xi[k] != 0.0)) fold = false;
     }
-    o.tb.r_on = d->taper_on; o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on);
+    o.tb.fold = fold ? 1 : 0;
+    for (size_t k = 0; k < nt2; ++k) {
+      const double pre_rho = d->xi[k] * d->xi[k], pre_rep = 2.0 * d->A[k];
+      o.tb.a_rho[k] = 2.0 * d->q[k] + (fold ? log(pre_rho) : 0.0); o.tb.b_rho[k] = 2.0 * d->q[k] / d->r0[k];
+      o.tb.a_rep[k] = d->p[k] + (fold ? log(pre_rep) : 0.0); o.tb.b_rep[k] = d->p[k] / d->r0[k];
+      o.tb.pre_rho[k] = fold ? 1.0 : pre_rho; o.tb.pre_rep[k] = fold ? 1.0 : pre_rep;
+      // exp_tab() has no overflow handling: its argument must stay well inside +-690 for 0 <= r <= r_c + skin
+      const double rmax = d->cutoff + d->skin;
+      if (!(fabs(o.tb.a_rho[k]) + fabs(o.tb.b_rho[k]) * rmax < 600.0) || !(fabs(o.tb.a_rep[k]) + fabs(o.tb.b_rep[k]) * rmax < 600.0)) {
+        delete s; return MD_EINVAL;
+      }
+    }
+    o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on); o.tb.t0 = -d->taper_on * o.tb.inv_w;
   } else {
     TableParams &t = o.tab;
     t.nr = d->nr; t.nrho = d->nrho; t.dr = d->dr; t.inv_dr = 1.0 / d->dr; t.drho = d->drho; t.inv_drho = 1.0 / d->drho;
@@ -351,6 +376,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     void *dst[6] = {(void *)t.f_val, (void *)t.f_der, (void *)t.phi_val, (void *)t.phi_der, (void *)t.F_val, (void *)t.F_der};
     for (int k = 0; k < 6 && e == cudaSuccess; ++k)
       e = cudaMemcpyAsync(dst[k], src[k], (k < 4 ? nt2 * d->nr : (size_t)o.nt * d->nrho) * sizeof(double), cudaMemcpyDefault, st);
+    if (e == cudaSuccess && launch_prepare_tables(s) != 0) e = cudaErrorUnknown;
   }
   // positions + types (through the staging area when they live on the host)
   const double *xdev = d->positions;

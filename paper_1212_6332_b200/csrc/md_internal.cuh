@@ -29,25 +29,32 @@ struct DevState {
 };
 
 struct TbsmaParams {               // per type pair, pre-combined on the host
-  double A2[kPairs];               // 2A
-  double xi2[kPairs];              // xi^2
-  double p[kPairs], p_r0[kPairs];  // p, p/r0
-  double q2[kPairs], q2_r0[kPairs];// 2q, 2q/r0
-  double r_on, inv_w;              // taper start, 1/(r_c - r_on)
+  // rho(r) = pre_rho exp(a_rho - b_rho r) S(r),  V(r) = pre_rep exp(a_rep - b_rep r) S(r)
+  // fold != 0: ln(xi^2) and ln(2A) are folded into a_rho / a_rep and pre_* = 1 (all prefactors > 0)
+  double a_rho[kPairs], b_rho[kPairs], pre_rho[kPairs];
+  double a_rep[kPairs], b_rep[kPairs], pre_rep[kPairs];
+  double inv_w, t0;                // switch variable t = clamp(r inv_w + t0, 0, 1): inv_w = 1/(r_c - r_on), t0 = -r_on inv_w
+  int fold;
 };
 
+// Cubic-Hermite tables re-expressed per INTERVAL k (r in [k dr, (k+1) dr), t = r/dr - k) at md_create:
+//   value      c0 + t (c1 + t (c2 + t c3))            c0 = y_k, c1 = h y'_k, c2 = 3D - h(2 y'_k + y'_{k+1}), c3 = h(y'_k + y'_{k+1}) - 2D
+//   derivative (c1 + t (2 c2 + 3 c3 t)) / h  =  d1 + t (d2 + t d3)
 struct TableParams {
   int nr, nrho;
   double dr, inv_dr, drho, inv_drho, rho_max;
-  const double *f_val, *f_der, *phi_val, *phi_der;   // [nt*nt][nr]
+  const double *f_val, *f_der, *phi_val, *phi_der;   // [nt*nt][nr]   node data as given (kept for the embedding and as the source)
   const double *F_val, *F_der;                       // [nt][nrho]
+  const double4 *f_c;                                // [nt*nt][nr-1]  (c0,c1,c2,c3) of rho(r): density pass
+  const double4 *phi_c;                              // [nt*nt][nr-1]  (c0,c1,c2,c3) of V(r): force pass with observables
+  const double4 *der_c;                              // [nt*nt][nr-1][2]  (fd1,fd2,fd3,0), (pd1,pd2,pd3,0): force pass
 };
 
 // Everything a kernel needs, passed by value as a __grid_constant__ parameter.
 struct DevSys {
   int N, nb, npb, nt;
   double L[3], hL[3];
-  double rc2, rl2, thr2;
+  double rc2, rl2, thr2, rin2;     // rin2: build-time split of a list row (pairs with r2 < rin2 first)
   int nc[3], tnc, ncell;           // cells per box (per dim, total) and cells of all boxes
   double cell_scale[3];            // nc/L
   int cap;                         // neighbour capacity per atom
@@ -62,7 +69,10 @@ struct DevSys {
   double4 *pos_tmp; double *vel_tmp; int *type_tmp, *orig_tmp;
   int *cell_id, *cell_count, *cell_start, *cell_fill, *perm, *scan_block;
   // neighbour list, blocked ELL: entry k of the atom in (tile, lane) at nbr[(tile*cap + k)*32 + lane]
+  // entries that were inside r_c at build time are at k = 0 .. n_in-1, the others at k = cap-n_out .. cap-1;
+  // ncount = n_in | n_out << 16
   unsigned *nbr; int *ncount;
+  const double *exp_tab;           // [64] 2^(j/64), correctly rounded (staged into shared memory by the passes)
   // per-atom results
   double *rho, *eemb, *eatom;
   double *partial;                 // [n_blocks][8] block partial sums: E, Wxx,Wyy,Wzz,Wxy,Wxz,Wyz, (pad)
@@ -98,6 +108,7 @@ inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block
 // launchers (each enqueues on s->stream; returns cudaError_t of the launch)
 int launch_rebuild_chain(md_system *s);                       // conditional on DevState (force_rebuild / maxd2)
 int launch_density(md_system *s);
+int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
 int launch_force(md_system *s, bool observables, double half_dt); // half_dt = dt/2 (0: no velocity update)
 int launch_kick_drift(md_system *s, double dt);
 int launch_reduce_boxes(md_system *s);

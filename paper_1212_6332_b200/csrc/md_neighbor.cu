@@ -194,7 +194,11 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   const int cz = cell_coord(pi.z, s.cell_scale[2], s.nc[2]);
   const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
   const int zlo = max(cz - 1, 0), zhi = min(cz + 1, ncz - 1);
-  int n = 0;
+  int n_all = 0;
+  bool overflow = false;
+  // pairs inside r_in (= r_c) now go to the front of the row (k = 0, 1, ...), skin pairs to the back (k = cap-1, cap-2, ...):
+  // the two passes run the full pair evaluation only over the front part (md_force.cu)
+  int n_in = 0, n_out = 0;
   for (int ox = -1; ox <= 1; ++ox) {
     int jx = cx + ox; jx += (jx < 0) ? ncx : 0; jx -= (jx >= ncx) ? ncx : 0;
     for (int oy = -1; oy <= 1; ++oy) {
@@ -215,18 +219,24 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           const double dz = min_image(__dsub_rn(pj.z, pi.z), s.L[2], s.hL[2], kz);
           const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
           if (r2 < s.rl2 && j != i) {
-            if (n < s.cap) row[(size_t)n * 32] = (unsigned)j | ((kx | (ky << 2) | (kz << 4)) << kIdxBits);
-            ++n;
+            const unsigned entry = (unsigned)j | ((kx | (ky << 2) | (kz << 4)) << kIdxBits);
+            if (n_in + n_out < s.cap) {
+              if (r2 < s.rin2) row[(size_t)(n_in++) * 32] = entry;
+              else row[(size_t)(s.cap - 1 - n_out++) * 32] = entry;
+            } else {
+              overflow = true;
+            }
+            ++n_all;
           }
         }
       }
     }
   }
-  if (n > s.cap) { atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW); }
-  s.ncount[i] = min(n, s.cap);
+  if (overflow) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
+  s.ncount[i] = n_in | (n_out << 16);
   // statistics: one atomic per warp
   const unsigned act = __activemask();
-  const int wsum = __reduce_add_sync(act, min(n, s.cap)), wmax = __reduce_max_sync(act, n);
+  const int wsum = __reduce_add_sync(act, n_in + n_out), wmax = __reduce_max_sync(act, n_all);
   if ((threadIdx.x & 31) == __ffs(act) - 1) {
     atomicAdd(&s.st->list_entries, (unsigned long long)wsum);
     atomicMax(&s.st->max_neighbors, wmax);
