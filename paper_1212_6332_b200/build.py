@@ -26,7 +26,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in deps)
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
-    cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *sources()]
+    extra = os.environ.get("MD_NVCC_EXTRA", "").split()          # e.g. -DMD_FORCE_MINB=5 (tuning knobs of md_force.cu)
+    cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *sources()]
     subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB
 

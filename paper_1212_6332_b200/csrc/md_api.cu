@@ -111,7 +111,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
     coef[0] = b.take<double4>(nt2 * (d->nr - 1)); coef[1] = b.take<double4>(nt2 * (d->nr - 1));
     coef[2] = b.take<double4>(2 * nt2 * (d->nr - 1));
   }
-  double *exp_tab = b.take<double>(64);
+  double *exp_tab = b.take<double>(kExpTabLen);
   void *stage = b.take<char>(g.stage_bytes);
   if (sys) {
     DevSys &o = sys->d;
@@ -221,14 +221,14 @@ __global__ void k_export_neighbors(const __grid_constant__ DevSys s, int first, 
   const int i = s.perm[first + a];
   const int box = i / s.npb, local = i - box * s.npb;
   const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
-  const unsigned *row = s.nbr + tile * s.cap * 32 + (local & 31);
+  const unsigned *row = s.nbr + nbr_row_offset(tile, s.cap, local & 31);
   const int c = s.ncount[i], n_in = c & 0xffff, n = n_in + (c >> 16);
   count[a] = n;
   if (n > stride) { atomicOr(overflow, 1); return; }
   int *out = list + (size_t)a * stride;
   for (int k = 0; k < n; ++k) {
     const int kk = k < n_in ? k : s.cap - 1 - (k - n_in);        // front part, then the skin part stored from the back
-    const int v = s.orig[row[(size_t)kk * 32] & kIdxMask];
+    const int v = s.orig[row[nbr_entry(kk)] & kIdxMask];
     int b = k - 1;
     while (b >= 0 && out[b] > v) { out[b + 1] = out[b]; --b; }
     out[b + 1] = v;
@@ -343,11 +343,9 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   cudaStream_t st = s->stream;
   cudaError_t e = cudaMemsetAsync(o.st, 0, sizeof(DevState), st);
   {
-    // 2^(j/64), j = 0..63, rounded from long double (64-bit mantissa): the table of exp_tab() in md_force.cu
-    double tab[64];
-    for (int j = 0; j < 64; ++j) tab[j] = (double)exp2l((long double)j / 64.0L);
-    if (e == cudaSuccess) e = cudaMemcpyAsync((void *)o.exp_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // tab is on this stack frame
+    // 2^(j/64), j = 0..63, rounded from long double (64-bit mantissa): the table of exp_scaled() in md_force.cu
+    for (int j = 0; j < 64; ++j) s->exp_tab_host[j] = (double)exp2l((long double)j / 64.0L);
+    for (int j = 64; j < kExpTabLen; ++j) s->exp_tab_host[j] = 0.0;
   }
   if (d->pot_kind == MD_POT_TBSMA) {
     bool fold = true;
@@ -358,16 +356,22 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     o.tb.fold = fold ? 1 : 0;
     for (size_t k = 0; k < nt2; ++k) {
       const double pre_rho = d->xi[k] * d->xi[k], pre_rep = 2.0 * d->A[k];
-      o.tb.a_rho[k] = 2.0 * d->q[k] + (fold ? log(pre_rho) : 0.0); o.tb.b_rho[k] = 2.0 * d->q[k] / d->r0[k];
-      o.tb.a_rep[k] = d->p[k] + (fold ? log(pre_rep) : 0.0); o.tb.b_rep[k] = d->p[k] / d->r0[k];
+      const long double K = 64.0L / logl(2.0L);       // exp_scaled() takes its argument in units of ln2/64
+      const long double a_rho = 2.0L * d->q[k] + (fold ? logl((long double)pre_rho) : 0.0L), a_rep = (long double)d->p[k] + (fold ? logl((long double)pre_rep) : 0.0L);
+      o.tb.b_rho[k] = 2.0 * d->q[k] / d->r0[k]; o.tb.b_rep[k] = d->p[k] / d->r0[k];
+      o.tb.ak_rho[k] = (double)(a_rho * K); o.tb.bk_rho[k] = (double)((long double)o.tb.b_rho[k] * K);
+      o.tb.ak_rep[k] = (double)(a_rep * K); o.tb.bk_rep[k] = (double)((long double)o.tb.b_rep[k] * K);
       o.tb.pre_rho[k] = fold ? 1.0 : pre_rho; o.tb.pre_rep[k] = fold ? 1.0 : pre_rep;
-      // exp_tab() has no overflow handling: its argument must stay well inside +-690 for 0 <= r <= r_c + skin
+      // exp_scaled() has no overflow handling: its argument must stay well inside +-690 for 0 <= r <= r_c + skin
       const double rmax = d->cutoff + d->skin;
-      if (!(fabs(o.tb.a_rho[k]) + fabs(o.tb.b_rho[k]) * rmax < 600.0) || !(fabs(o.tb.a_rep[k]) + fabs(o.tb.b_rep[k]) * rmax < 600.0)) {
+      if (!(fabsl(a_rho) + fabs(o.tb.b_rho[k]) * rmax < 600.0) || !(fabsl(a_rep) + fabs(o.tb.b_rep[k]) * rmax < 600.0)) {
         delete s; return MD_EINVAL;
       }
     }
-    o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on); o.tb.t0 = -d->taper_on * o.tb.inv_w;
+    o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on); o.tb.t0 = -d->taper_on * o.tb.inv_w; o.tb.m30_inv_w = -30.0 * o.tb.inv_w;
+    // loop constants that the passes read from memory into registers (md_force.cu, LoopConsts)
+    double *lc = s->exp_tab_host + 64;
+    lc[0] = 1.0 / 120.0; lc[1] = 0.375; lc[2] = 6.0; lc[3] = o.tb.inv_w; lc[4] = o.tb.bk_rho[0]; lc[5] = o.tb.bk_rep[0];
   } else {
     TableParams &t = o.tab;
     t.nr = d->nr; t.nrho = d->nrho; t.dr = d->dr; t.inv_dr = 1.0 / d->dr; t.drho = d->drho; t.inv_drho = 1.0 / d->drho;
@@ -378,6 +382,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
       e = cudaMemcpyAsync(dst[k], src[k], (k < 4 ? nt2 * d->nr : (size_t)o.nt * d->nrho) * sizeof(double), cudaMemcpyDefault, st);
     if (e == cudaSuccess && launch_prepare_tables(s) != 0) e = cudaErrorUnknown;
   }
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void *)o.exp_tab, s->exp_tab_host, sizeof(s->exp_tab_host), cudaMemcpyHostToDevice, st);
   // positions + types (through the staging area when they live on the host)
   const double *xdev = d->positions;
   const int *tdev = d->types;

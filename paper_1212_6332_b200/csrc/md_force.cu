@@ -20,6 +20,17 @@
 
 namespace md {
 
+#ifndef MD_PAIR2
+#define MD_PAIR2 1
+#endif
+#ifndef MD_FORCE_MINB
+#define MD_FORCE_MINB 5
+#endif
+#ifndef MD_DENS_MINB
+#define MD_DENS_MINB 6
+#endif
+constexpr int kForceMinBlocks = MD_FORCE_MINB, kDensityMinBlocks = MD_DENS_MINB;
+
 // ------------------------------------------------------------------------------------------------
 // arithmetic helpers
 // ------------------------------------------------------------------------------------------------
@@ -31,6 +42,10 @@ __device__ __forceinline__ double image_delta(double xj, double xi, unsigned cod
   return d;
 }
 
+// CANON: r2 = (dx*dx + dy*dy) + dz*dz with every operation rounded once (reading A3), needed where r2 < rc2 decides a
+// discontinuous term (tables, reading A9).  Otherwise (TB-SMA: the clamped switch makes the term continuous and exactly 0
+// beyond r_c) two of the five operations are contracted into FMAs.
+template <bool CANON>
 __device__ __forceinline__ double pair_r2(const double4 &pj, const double4 &pi, unsigned e, const DevSys &s,
                                           double &dx, double &dy, double &dz) {
   const unsigned code = e >> kIdxBits;
@@ -41,49 +56,127 @@ __device__ __forceinline__ double pair_r2(const double4 &pj, const double4 &pi, 
     dy = image_delta(pj.y, pi.y, (code >> 2) & 3u, s.L[1]);
     dz = image_delta(pj.z, pi.z, (code >> 4) & 3u, s.L[2]);
   }
-  return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  if (CANON) return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  return fma(dz, dz, fma(dy, dy, dx * dx));
+}
+
+// An FP64 instruction takes at most ONE operand that is not a register (an immediate with a zero low word, or a
+// constant-bank address).  Constants that meet another constant in the same FMA are therefore read from MEMORY into
+// registers before the loop (LoopConsts): ptxas cannot rematerialise a global load, so they stay in registers instead
+// of being rebuilt by MOV / LDC pairs for every pair.  The others sit in the constant bank and are used in place.
+__constant__ double kLn2_64 = 0x1.62e42fefa39efp-7;           // ln2/64
+__constant__ double kC3 = 1.0 / 6.0, kC4 = 1.0 / 24.0;
+
+struct LoopConsts { double c5, c375, six, inv_w, bk_rho, bk_rep; };
+
+__device__ __forceinline__ double lds_opaque(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ LoopConsts load_loop_consts(unsigned tab) {   // tab = shared-space address of the staged exp_tab
+  LoopConsts c;
+  c.c5 = lds_opaque(tab + 512); c.c375 = lds_opaque(tab + 520); c.six = lds_opaque(tab + 528);
+  c.inv_w = lds_opaque(tab + 536); c.bk_rho = lds_opaque(tab + 544); c.bk_rep = lds_opaque(tab + 552);
+  return c;
 }
 
 // 1/sqrt(x), x > 0 finite and normal: hardware seed (relative error ~2^-22) and one cubic Newton step
 //   y1 = y (1 + e/2 + 3 e^2/8),  e = 1 - x y^2        (relative error 2.5 delta^3 ~ 2^-64 plus rounding)
-__device__ __forceinline__ double rsqrt_fast(double x) {
+__device__ __forceinline__ double rsqrt_fast(double x, double c375) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   const double e = fma(-x, y * y, 1.0);
-  const double p = fma(e, 0.375, 0.5);
+  const double p = fma(e, c375, 0.5);
   return fma(p, y * e, y);
 }
 
-// exp(x) for |x| < 690, no special cases.  n = rint(64 x / ln 2); r = x - n ln2/64, |r| <= 0.00542;
-// exp(x) = 2^(n >> 6) tab[n & 63] (1 + r + r^2/2 + r^3/6 + r^4/24 + r^5/120); remainder r^6/720 < 3.5e-17.
-__device__ __forceinline__ double exp_tab(double x, const double *__restrict__ tab) {
+// exp(xk ln2/64) for |xk ln2/64| < 690, no special cases; xk is the exponent in units of ln2/64.
+// n = rint(xk) (magic-number rounding); d = xk - n exactly, |d| <= 1/2; r = d ln2/64, |r| <= 0.00542;
+// result = 2^(n >> 6) tab[n & 63] (1 + r + r^2/2 + r^3/6 + r^4/24 + r^5/120); remainder r^6/720 < 3.5e-17.
+__device__ __forceinline__ double exp_scaled(double xk, unsigned tab, double c5) {   // tab = shared-space address of the table
   constexpr double kMagic = 6755399441055744.0;                 // 1.5 * 2^52: the low word of t holds n
-  const double t = fma(x, 0x1.71547652b82fep+6, kMagic);
+  const double t = xk + kMagic;
   const double n = t - kMagic;
-  double r = fma(n, -0x1.62e42fee00000p-7, x);                  // ln2/64, high 32 bits: n * hi is exact
-  r = fma(n, -0x1.a39ef35793c76p-39, r);
+  const double r = (xk - n) * kLn2_64;
   const int ni = __double2loint(t);
-  const double T = tab[ni & 63];
-  double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-  p = fma(p, r, 1.0 / 6.0);
+  double T;
+  asm("ld.shared.f64 %0, [%1];" : "=d"(T) : "r"(tab + ((unsigned)(ni & 63) << 3)));
+  double p = fma(r, c5, kC4);
+  p = fma(p, r, kC3);
   p = fma(p, r, 0.5);
   p = fma(p * r, r, r);
   const double v = fma(T, p, T);
   return __hiloint2double(__double2hiint(v) + ((ni >> 6) << 20), __double2loint(v));
 }
 
-// quintic switch on t in [0,1] (clamped): S = 1 - t^3 (10 - 15 t + 6 t^2), dS/dr = -30 t^2 (1-t)^2 inv_w.
-// t <= 0 gives S = 1, dS = 0 and t >= 1 gives S = 0, dS = 0 exactly.
-__device__ __forceinline__ double switch_t(double r, const TbsmaParams &tb) {
-  return fmin(fmax(fma(r, tb.inv_w, tb.t0), 0.0), 1.0);
+// The same arithmetic for NP pairs at once, written step by step across the pairs: ptxas keeps roughly the source order,
+// so the NP dependency chains end up interleaved in the instruction stream (rsqrt_fast / exp_scaled / switch_* above
+// are the single-pair forms of exactly these steps).
+#define MD_EACH for (int q = 0; q < NP; ++q)
+template <int NP>
+__device__ __forceinline__ void rsqrt_fast_n(const double (&x)[NP], double c375, double (&y)[NP]) {
+  double e[NP], p[NP], ye[NP];
+#pragma unroll
+  MD_EACH asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[q]) : "d"(x[q]));
+#pragma unroll
+  MD_EACH e[q] = y[q] * y[q];
+#pragma unroll
+  MD_EACH e[q] = fma(-x[q], e[q], 1.0);
+#pragma unroll
+  MD_EACH p[q] = fma(e[q], c375, 0.5);
+#pragma unroll
+  MD_EACH ye[q] = y[q] * e[q];
+#pragma unroll
+  MD_EACH y[q] = fma(p[q], ye[q], y[q]);
 }
-__device__ __forceinline__ double switch_S(double t) {
+
+template <int NP>
+__device__ __forceinline__ void exp_scaled_n(const double (&xk)[NP], unsigned tab, double c5, double (&out)[NP]) {
+  constexpr double kMagic = 6755399441055744.0;
+  double t[NP], n[NP], r[NP], T[NP], p[NP];
+  int ni[NP];
+#pragma unroll
+  MD_EACH t[q] = xk[q] + kMagic;
+#pragma unroll
+  MD_EACH { n[q] = t[q] - kMagic; ni[q] = __double2loint(t[q]); }
+#pragma unroll
+  MD_EACH {
+    asm("ld.shared.f64 %0, [%1];" : "=d"(T[q]) : "r"(tab + ((unsigned)(ni[q] & 63) << 3)));
+  }
+#pragma unroll
+  MD_EACH r[q] = (xk[q] - n[q]) * kLn2_64;
+#pragma unroll
+  MD_EACH p[q] = fma(r[q], c5, kC4);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], kC3);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], 0.5);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q] * r[q], r[q], r[q]);
+#pragma unroll
+  MD_EACH {
+    const double v = fma(T[q], p[q], T[q]);
+    out[q] = __hiloint2double(__double2hiint(v) + ((ni[q] >> 6) << 20), __double2loint(v));
+  }
+}
+
+// quintic switch on t in [0,1]: S = 1 - t^3 (10 - 15 t + 6 t^2), dS/dr = -30 t^2 (1-t)^2 inv_w.
+// switch_t clamps on the high word with integer min/max (no FP64-pipe instruction): t <= 0 gives t = 0 (S = 1,
+// dS = 0 exactly) and t >= 1 gives t = 1 (S = 0, dS = 0 exactly).
+__device__ __forceinline__ double switch_t(double r, double inv_w, double t0) {
+  const double t = fma(r, inv_w, t0);
+  const int hi = __double2hiint(t);
+  const int hc = min(max(hi, 0), 0x3ff00000);
+  return __hiloint2double(hc, (unsigned)hi < 0x3ff00000u ? __double2loint(t) : 0);
+}
+__device__ __forceinline__ double switch_S(double t, double six) {
   const double t2 = t * t;
-  return fma(-(t2 * t), fma(t, fma(t, 6.0, -15.0), 10.0), 1.0);
+  return fma(-(t2 * t), fma(t, fma(t, six, -15.0), 10.0), 1.0);
 }
-__device__ __forceinline__ double switch_dS(double t, double inv_w) {
+__device__ __forceinline__ double switch_dS(double t, double m30_inv_w) {
   const double u = 1.0 - t, tu = t * u;
-  return (-30.0 * inv_w) * (tu * tu);
+  return m30_inv_w * (tu * tu);
 }
 
 // cubic Hermite from NODE data (embedding function only: once per atom)
@@ -132,71 +225,129 @@ __device__ __forceinline__ void embed(const DevSys &s, int ti, double rho, doubl
 }
 
 // ------------------------------------------------------------------------------------------------
-// list row walkers.  Row of the atom in (tile, lane): entry k at row[k*32].  Entries 0 .. n_in-1 were inside
-// r_c at build time ("main"), entries cap-n_out .. cap-1 were in the skin ("tail").  Both walkers keep the
-// entry of pair k+2 and the gathered position of pair k+1 in flight while pair k is evaluated.
+// list row walkers.  The row of the atom in (tile, lane) is a sequence of 16-byte groups of four entries, group g
+// at row[g * 32] (uint4 units).  Entries 0 .. n_in-1 were inside r_c at build time ("main"), entries cap-n_out ..
+// cap-1 were in the skin ("tail").  A walker keeps the entries of the next TWO groups and the gathered position of
+// the next pair in flight while a pair is evaluated: the list is a DRAM stream (latency ~1 us), the gathers hit L1/L2.
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 ldg_group(const uint4 *p) { return __ldg(p); }
+#define MD_GIDX(e) ((e) & kIdxMask)
+
+// One 256-bit load per gathered neighbour (LDG.E.256, sm_100): both passes are bound by the L1 data pipe, and a
+// 32-byte gather issued as two 128-bit loads costs twice the wavefronts.
+__device__ __forceinline__ double4 gather32(const double4 *p) {
+  double4 v;
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
+}
+
+// body2 evaluates two pairs at once: their dependency chains are independent, which is what lets the FP64 pipe run near
+// its issue rate at the 4-5 resident warps per scheduler that the register budget allows (measured on B200: one
+// dependent DFMA chain per warp tops out at 64 % of the pipe, two at 77 %, four at 90 %).
+template <class Body2, class Body1>
+__device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, const double4 *__restrict__ pos, Body2 body2, Body1 body1) {
+  const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+  const int ng = (n + 3) >> 2, nfull = n >> 2;
+  uint4 E = ng > 0 ? ldg_group(row) : zero;
+  uint4 En = ng > 1 ? ldg_group(row + 32) : zero;
+  double4 pA = gather32(pos + MD_GIDX(E.x));                      // slot 0 when there is no such pair: harmless
+  double4 pB = gather32(pos + MD_GIDX(E.y));
+#if MD_PAIR2
+  for (int g = 0; g < nfull; ++g) {
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : zero;
+    const double4 pC = gather32(pos + MD_GIDX(E.z));
+    const double4 pD = gather32(pos + MD_GIDX(E.w));
+    body2(E.x, pA, E.y, pB);
+    pA = gather32(pos + MD_GIDX(En.x));
+    pB = gather32(pos + MD_GIDX(En.y));
+    body2(E.z, pC, E.w, pD);
+    E = En; En = E2;
+  }
+  const int rem = n & 3;                                          // the partly filled last group
+  if (rem >= 2) {
+    const double4 pC = gather32(pos + MD_GIDX(E.z));
+    body2(E.x, pA, E.y, pB);
+    if (rem == 3) body1(E.z, pC);
+  } else if (rem == 1) {
+    body1(E.x, pA);
+  }
+#else
+  for (int g = 0; g < nfull; ++g) {
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : zero;
+    const double4 pC = gather32(pos + MD_GIDX(E.z));
+    body1(E.x, pA);
+    const double4 pD = gather32(pos + MD_GIDX(E.w));
+    body1(E.y, pB);
+    pA = gather32(pos + MD_GIDX(En.x));
+    body1(E.z, pC);
+    pB = gather32(pos + MD_GIDX(En.y));
+    body1(E.w, pD);
+    E = En; En = E2;
+  }
+  const int rem = n & 3;
+  if (rem >= 1) body1(E.x, pA);
+  if (rem >= 2) body1(E.y, pB);
+  if (rem == 3) { const double4 pC = gather32(pos + MD_GIDX(E.z)); body1(E.z, pC); }
+#endif
+}
+
+// Tail: walked from the END of the row (entry cap-1-j, j = 0 .. n-1), so that every lane starts on a group boundary.
+// last = the last group of the row; mg = warp-uniform number of groups (max over the warp of ceil(n/4));
+// body(e, pj, active) is called by all 32 lanes.
 template <class Body>
-__device__ __forceinline__ void walk_main(const unsigned *__restrict__ row, int n, const double4 *__restrict__ pos, Body body) {
-  unsigned e_nx = n > 0 ? row[0] : 0u;
-  unsigned e_n2 = n > 1 ? row[32] : 0u;
-  double4 p_nx = pos[e_nx & kIdxMask];
-  for (int k = 0; k < n; ++k) {
-    const unsigned e = e_nx;
-    const double4 pj = p_nx;
-    e_nx = e_n2;
-    p_nx = pos[e_nx & kIdxMask];                               // slot 0 when there is no next pair: harmless
-    e_n2 = (k + 2 < n) ? row[(size_t)(k + 2) * 32] : 0u;
-    body(e, pj);
+__device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n, int mg, const double4 *__restrict__ pos, Body body) {
+  const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+  const int ng = (n + 3) >> 2;
+  uint4 E = ng > 0 ? ldg_group(last) : zero;
+  uint4 En = ng > 1 ? ldg_group(last - 32) : zero;
+  double4 pA = gather32(pos + MD_GIDX(E.w));
+  for (int g = 0; g < mg; ++g) {
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32) : zero;
+    const int j = g * 4;
+    const double4 pB = gather32(pos + MD_GIDX(E.z));
+    body(E.w, pA, j < n);
+    const double4 pC = gather32(pos + MD_GIDX(E.y));
+    body(E.z, pB, j + 1 < n);
+    const double4 pD = gather32(pos + MD_GIDX(E.x));
+    body(E.y, pC, j + 2 < n);
+    pA = gather32(pos + MD_GIDX(En.w));
+    body(E.x, pD, j + 3 < n);
+    E = En; En = E2;
   }
 }
 
-// m = warp-uniform trip count (max of n over the warp); body(e, pj, active) is called by all 32 lanes
-template <class Body>
-__device__ __forceinline__ void walk_tail(const unsigned *__restrict__ row, int n, int m, const double4 *__restrict__ pos, Body body) {
-  unsigned e_nx = n > 0 ? row[0] : 0u;
-  unsigned e_n2 = n > 1 ? row[32] : 0u;
-  double4 p_nx = pos[e_nx & kIdxMask];
-  for (int k = 0; k < m; ++k) {
-    const unsigned e = e_nx;
-    const double4 pj = p_nx;
-    e_nx = e_n2;
-    p_nx = pos[e_nx & kIdxMask];
-    e_n2 = (k + 2 < n) ? row[(size_t)(k + 2) * 32] : 0u;
-    body(e, pj, k < n);
-  }
-}
-
-struct AtomRow { const unsigned *main, *tail; int n_in, n_out; };
+struct AtomRow { const uint4 *main, *last; int n_in, n_out; };
 
 __device__ __forceinline__ AtomRow atom_row(const DevSys &s, int box, int local, int i, bool valid) {
   AtomRow r;
   const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
-  r.main = s.nbr + tile * s.cap * 32 + (local & 31);
+  r.main = (const uint4 *)(s.nbr + nbr_row_offset(tile, s.cap, local & 31));
   const int c = valid ? s.ncount[i] : 0;
   r.n_in = c & 0xffff; r.n_out = c >> 16;
-  r.tail = r.main + (size_t)(s.cap - r.n_out) * 32;
+  r.last = r.main + (size_t)((s.cap >> 2) - 1) * 32;
   return r;
 }
 
-__device__ __forceinline__ void stage_exp_table(const DevSys &s, double *tab) {
-  if (threadIdx.x < 64) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
+__device__ __forceinline__ unsigned stage_exp_table(const DevSys &s, double *tab) {
+  if (threadIdx.x < kExpTabLen) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
   __syncthreads();
+  return (unsigned)__cvta_generic_to_shared(tab);
 }
 
 // ------------------------------------------------------------------------------------------------
 // Density pass: rho_i = sum_{j in list, r2 < rc2} rho(r_ij); F(rho_i), F'(rho_i).
 // ------------------------------------------------------------------------------------------------
-template <int KIND, bool FOLD>
-__device__ __forceinline__ double density_term(const DevSys &s, const double *tab, int tp, double r2) {
-  const double r = r2 * rsqrt_fast(r2);
+template <int KIND, bool MULTI, bool FOLD>
+__device__ __forceinline__ double density_term(const DevSys &s, const LoopConsts &lc, unsigned tab, int tp, double r2) {
   if (KIND == MD_POT_TBSMA) {
     const TbsmaParams &tb = s.tb;
-    const double S = switch_S(switch_t(r, tb));
-    double e = exp_tab(fma(-tb.b_rho[tp], r, tb.a_rho[tp]), tab);
+    const double r = r2 * rsqrt_fast(r2, lc.c375);
+    const double S = switch_S(switch_t(r, lc.inv_w, tb.t0), lc.six);
+    double e = exp_scaled(fma(-(MULTI ? tb.bk_rho[tp] : lc.bk_rho), r, tb.ak_rho[tp]), tab, lc.c5);
     if (!FOLD) e *= tb.pre_rho[tp];
     return e * S;
   } else {
+    const double r = r2 * rsqrt_fast(r2, 0.375);
     double t;
     const int k = table_index(s.tab, r, t);
     const double4 c = ldg4(s.tab.f_c + (size_t)tp * (s.tab.nr - 1) + k);
@@ -204,10 +355,29 @@ __device__ __forceinline__ double density_term(const DevSys &s, const double *ta
   }
 }
 
+template <bool FOLD, int NP>
+__device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts &lc, unsigned tab, const double (&r2)[NP], double (&term)[NP]) {
+  const TbsmaParams &tb = s.tb;
+  double rinv[NP], r[NP], t[NP], xh[NP], eh[NP];
+  rsqrt_fast_n<NP>(r2, lc.c375, rinv);
+#pragma unroll
+  MD_EACH r[q] = r2[q] * rinv[q];
+#pragma unroll
+  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0); }
+  exp_scaled_n<NP>(xh, tab, lc.c5, eh);
+#pragma unroll
+  MD_EACH {
+    if (!FOLD) eh[q] *= tb.pre_rho[0];
+    term[q] = eh[q] * switch_S(t[q], lc.six);
+  }
+}
+
 template <int KIND, bool MULTI, bool FOLD>
-__global__ void __launch_bounds__(kForceBlock) k_density(const __grid_constant__ DevSys s) {
-  __shared__ double tab[64];
-  if (KIND == MD_POT_TBSMA) stage_exp_table(s, tab);
+__global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s) {
+  __shared__ double tab_sm[kExpTabLen];
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
@@ -215,34 +385,55 @@ __global__ void __launch_bounds__(kForceBlock) k_density(const __grid_constant__
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.pos[i];
   const int ti = MULTI ? (int)pi.w : 0;
-  double rho = 0.0;
+  double rho = 0.0, rho2 = 0.0;
 
   // main part: branch-free.  TB-SMA: the clamped switch makes a pair beyond r_c contribute exactly 0;
   // tables (no switch, reading A9): the strict test r2 < rc2 selects the term.
-  walk_main(row.main, row.n_in, s.pos, [&](unsigned e, const double4 &pj) {
-    double dx, dy, dz;
-    const double r2 = pair_r2(pj, pi, e, s, dx, dy, dz);
-    const int tp = MULTI ? ti * s.nt + (int)pj.w : 0;
-    const double term = density_term<KIND, FOLD>(s, tab, tp, r2);
+  auto add1 = [&](double r2, int tp) {
+    const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, tp, r2);
     if (KIND == MD_POT_TBSMA) rho += term;
     else rho += (r2 < s.rc2) ? term : 0.0;
-  });
+  };
+  walk_main(row.main, row.n_in, s.pos,
+            [&](unsigned eA, const double4 &pA, unsigned eB, const double4 &pB) {
+              double dx, dy, dz;
+              const double r2A = pair_r2<KIND != MD_POT_TBSMA>(pA, pi, eA, s, dx, dy, dz);
+              const double r2B = pair_r2<KIND != MD_POT_TBSMA>(pB, pi, eB, s, dx, dy, dz);
+              double tA, tB;
+              if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
+                const double r2v[2] = {r2A, r2B};
+                double tv[2];
+                density_term_n<FOLD, 2>(s, lc, tab, r2v, tv);
+                tA = tv[0]; tB = tv[1];
+              } else {
+                tA = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pA.w : 0, r2A);
+                tB = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pB.w : 0, r2B);
+              }
+              if (KIND == MD_POT_TBSMA) { rho += tA; rho2 += tB; }
+              else { rho += (r2A < s.rc2) ? tA : 0.0; rho2 += (r2B < s.rc2) ? tB : 0.0; }
+            },
+            [&](unsigned e, const double4 &pj) {
+              double dx, dy, dz;
+              const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
+              add1(r2, MULTI ? ti * s.nt + (int)pj.w : 0);
+            });
+  rho += rho2;
 
   // skin part: distance test only; a pair found inside r_c is parked (one slot per lane) and the warp evaluates
   // the parked pairs together when some lane needs its slot again, and once at the end
-  const int m = __reduce_max_sync(0xffffffffu, row.n_out);
+  const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
   double park_r2 = 0.0; int park_tp = 0; bool parked = false;
-  walk_tail(row.tail, row.n_out, m, s.pos, [&](unsigned e, const double4 &pj, bool active) {
+  walk_tail(row.last, row.n_out, mg, s.pos, [&](unsigned e, const double4 &pj, bool active) {
     double dx, dy, dz;
-    const double r2 = pair_r2(pj, pi, e, s, dx, dy, dz);
+    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
     const bool hit = active && r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
-      if (parked) { rho += density_term<KIND, FOLD>(s, tab, park_tp, park_r2); parked = false; }
+      if (parked) { rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, park_tp, park_r2); parked = false; }
     }
     if (hit) { park_r2 = r2; park_tp = MULTI ? ti * s.nt + (int)pj.w : 0; parked = true; }
   });
   if (__any_sync(0xffffffffu, parked)) {
-    if (parked) rho += density_term<KIND, FOLD>(s, tab, park_tp, park_r2);
+    if (parked) rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, park_tp, park_r2);
   }
 
   if (!valid) return;
@@ -266,21 +457,23 @@ template <> struct ForceAcc<false> { double fx = 0.0, fy = 0.0, fz = 0.0; };
 template <> struct ForceAcc<true> { double fx = 0.0, fy = 0.0, fz = 0.0, ev = 0.0, w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0, w4 = 0.0, w5 = 0.0; };
 
 // g = s_ij / r and V for one pair; `in` = the pair is inside r_c (only consulted for the tables)
-template <int KIND, bool OBS, bool FOLD>
-__device__ __forceinline__ void force_term(const DevSys &s, const double *tab, int tp, double r2, double fp_sum, double &g, double &V) {
-  const double rinv = rsqrt_fast(r2), r = r2 * rinv;
+template <int KIND, bool MULTI, bool OBS, bool FOLD>
+__device__ __forceinline__ void force_term(const DevSys &s, const LoopConsts &lc, unsigned tab, int tp, double r2, double fp_sum,
+                                           double &g, double &V) {
   if (KIND == MD_POT_TBSMA) {
     const TbsmaParams &tb = s.tb;
-    const double t = switch_t(r, tb);
-    const double S = switch_S(t), dS = switch_dS(t, tb.inv_w);
-    double eh = exp_tab(fma(-tb.b_rho[tp], r, tb.a_rho[tp]), tab);
-    double er = exp_tab(fma(-tb.b_rep[tp], r, tb.a_rep[tp]), tab);
+    const double rinv = rsqrt_fast(r2, lc.c375), r = r2 * rinv;
+    const double t = switch_t(r, lc.inv_w, tb.t0);
+    const double S = switch_S(t, lc.six), dS = switch_dS(t, tb.m30_inv_w);
+    double eh = exp_scaled(fma(-(MULTI ? tb.bk_rho[tp] : lc.bk_rho), r, tb.ak_rho[tp]), tab, lc.c5);
+    double er = exp_scaled(fma(-(MULTI ? tb.bk_rep[tp] : lc.bk_rep), r, tb.ak_rep[tp]), tab, lc.c5);
     if (!FOLD) { eh *= tb.pre_rho[tp]; er *= tb.pre_rep[tp]; }
     const double df = eh * fma(-tb.b_rho[tp], S, dS);
     const double dV = er * fma(-tb.b_rep[tp], S, dS);
     g = fma(fp_sum, df, dV) * rinv;
     if (OBS) V = er * S;
   } else {
+    const double rinv = rsqrt_fast(r2, 0.375), r = r2 * rinv;
     double t;
     const int k = table_index(s.tab, r, t);
     const size_t o = (size_t)tp * (s.tab.nr - 1) + k;
@@ -289,6 +482,31 @@ __device__ __forceinline__ void force_term(const DevSys &s, const double *tab, i
     const double dV = fma(t, fma(t, cp.z, cp.y), cp.x);
     g = fma(fp_sum, df, dV) * rinv;
     if (OBS) { const double4 c = ldg4(s.tab.phi_c + o); V = fma(t, fma(t, fma(t, c.w, c.z), c.y), c.x); }
+  }
+}
+
+// NP pairs at once (TB-SMA, one type pair): the steps of force_term, interleaved across the pairs
+template <bool OBS, bool FOLD, int NP>
+__device__ __forceinline__ void force_term_n(const DevSys &s, const LoopConsts &lc, unsigned tab, const double (&r2)[NP],
+                                             const double (&fp_sum)[NP], double (&g)[NP], double (&V)[NP]) {
+  const TbsmaParams &tb = s.tb;
+  double rinv[NP], r[NP], t[NP], S[NP], dS[NP], xh[NP], xr[NP], eh[NP], er[NP];
+  rsqrt_fast_n<NP>(r2, lc.c375, rinv);
+#pragma unroll
+  MD_EACH r[q] = r2[q] * rinv[q];
+#pragma unroll
+  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); xr[q] = fma(-lc.bk_rep, r[q], tb.ak_rep[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0); }
+  exp_scaled_n<NP>(xh, tab, lc.c5, eh);
+  exp_scaled_n<NP>(xr, tab, lc.c5, er);
+#pragma unroll
+  MD_EACH { S[q] = switch_S(t[q], lc.six); dS[q] = switch_dS(t[q], tb.m30_inv_w); }
+#pragma unroll
+  MD_EACH {
+    if (!FOLD) { eh[q] *= tb.pre_rho[0]; er[q] *= tb.pre_rep[0]; }
+    const double df = eh[q] * fma(-tb.b_rho[0], S[q], dS[q]);
+    const double dV = er[q] * fma(-tb.b_rep[0], S[q], dS[q]);
+    g[q] = fma(fp_sum[q], df, dV) * rinv[q];
+    if (OBS) V[q] = er[q] * S[q];
   }
 }
 
@@ -303,11 +521,19 @@ __device__ __forceinline__ void force_accumulate(ForceAcc<OBS> &a, double g, dou
   }
 }
 
+template <bool OBS>
+__device__ __forceinline__ void force_merge(ForceAcc<OBS> &a, const ForceAcc<OBS> &b) {
+  a.fx += b.fx; a.fy += b.fy; a.fz += b.fz;
+  if constexpr (OBS) { a.ev += b.ev; a.w0 += b.w0; a.w1 += b.w1; a.w2 += b.w2; a.w3 += b.w3; a.w4 += b.w4; a.w5 += b.w5; }
+}
+
 template <int KIND, bool MULTI, bool OBS, bool FOLD>
-__global__ void __launch_bounds__(kForceBlock) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
-  __shared__ double tab[64];
+__global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
+  __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
-  if (KIND == MD_POT_TBSMA) stage_exp_table(s, tab);
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
@@ -315,28 +541,51 @@ __global__ void __launch_bounds__(kForceBlock) k_force(const __grid_constant__ D
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.posf[i];
   const int ti = MULTI ? s.type[i] : 0;
-  ForceAcc<OBS> acc;
+  ForceAcc<OBS> acc, acc2;
 
-  walk_main(row.main, row.n_in, s.posf, [&](unsigned e, const double4 &pj) {
-    double dx, dy, dz, g, V = 0.0;
-    const double r2 = pair_r2(pj, pi, e, s, dx, dy, dz);
-    const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
-    force_term<KIND, OBS, FOLD>(s, tab, tp, r2, pi.w + pj.w, g, V);
-    if (KIND != MD_POT_TBSMA && !(r2 < s.rc2)) { g = 0.0; V = 0.0; }   // tables: strict cut-off, no switch (reading A9)
-    force_accumulate<OBS>(acc, g, V, dx, dy, dz);
-  });
+  walk_main(row.main, row.n_in, s.posf,
+            [&](unsigned eA, const double4 &pA, unsigned eB, const double4 &pB) {
+              double dxA, dyA, dzA, dxB, dyB, dzB, gA, gB, VA = 0.0, VB = 0.0;
+              const double r2A = pair_r2<KIND != MD_POT_TBSMA>(pA, pi, eA, s, dxA, dyA, dzA);
+              const double r2B = pair_r2<KIND != MD_POT_TBSMA>(pB, pi, eB, s, dxB, dyB, dzB);
+              if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
+                const double r2v[2] = {r2A, r2B}, fpv[2] = {pi.w + pA.w, pi.w + pB.w};
+                double gv[2], Vv[2] = {0.0, 0.0};
+                force_term_n<OBS, FOLD, 2>(s, lc, tab, r2v, fpv, gv, Vv);
+                gA = gv[0]; gB = gv[1]; VA = Vv[0]; VB = Vv[1];
+              } else {
+                const int tpA = MULTI ? ti * s.nt + s.type[eA & kIdxMask] : 0, tpB = MULTI ? ti * s.nt + s.type[eB & kIdxMask] : 0;
+                force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tpA, r2A, pi.w + pA.w, gA, VA);
+                force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tpB, r2B, pi.w + pB.w, gB, VB);
+              }
+              if (KIND != MD_POT_TBSMA) {                          // tables: strict cut-off, no switch (reading A9)
+                if (!(r2A < s.rc2)) { gA = 0.0; VA = 0.0; }
+                if (!(r2B < s.rc2)) { gB = 0.0; VB = 0.0; }
+              }
+              force_accumulate<OBS>(acc, gA, VA, dxA, dyA, dzA);
+              force_accumulate<OBS>(acc2, gB, VB, dxB, dyB, dzB);
+            },
+            [&](unsigned e, const double4 &pj) {
+              double dx, dy, dz, g, V = 0.0;
+              const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
+              const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
+              force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, r2, pi.w + pj.w, g, V);
+              if (KIND != MD_POT_TBSMA && !(r2 < s.rc2)) { g = 0.0; V = 0.0; }
+              force_accumulate<OBS>(acc, g, V, dx, dy, dz);
+            });
+  force_merge<OBS>(acc, acc2);
 
-  const int m = __reduce_max_sync(0xffffffffu, row.n_out);
+  const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
   double pk_dx = 0.0, pk_dy = 0.0, pk_dz = 0.0, pk_r2 = 1.0, pk_fp = 0.0; int pk_tp = 0; bool parked = false;
   auto flush = [&]() {
     double g, V = 0.0;
-    force_term<KIND, OBS, FOLD>(s, tab, pk_tp, pk_r2, pk_fp, g, V);
+    force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, pk_tp, pk_r2, pk_fp, g, V);
     force_accumulate<OBS>(acc, g, V, pk_dx, pk_dy, pk_dz);
     parked = false;
   };
-  walk_tail(row.tail, row.n_out, m, s.posf, [&](unsigned e, const double4 &pj, bool active) {
+  walk_tail(row.last, row.n_out, mg, s.posf, [&](unsigned e, const double4 &pj, bool active) {
     double dx, dy, dz;
-    const double r2 = pair_r2(pj, pi, e, s, dx, dy, dz);
+    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
     const bool hit = active && r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
       if (parked) flush();

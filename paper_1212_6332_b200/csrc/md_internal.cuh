@@ -14,6 +14,7 @@ constexpr int kIdxBits = 26;                       // neighbour entry = index | 
 constexpr unsigned kIdxMask = (1u << kIdxBits) - 1u;
 constexpr int kMaxAtoms = 1 << kIdxBits;
 constexpr int kPairs = MD_MAX_TYPES * MD_MAX_TYPES;
+constexpr int kExpTabLen = 64 + 8;                  // 2^(j/64) table + the loop constants of the passes (md_force.cu)
 constexpr double kAmuToEvFs2PerA2 = 103.642696526805;  // 1 amu (A/fs)^2 in eV
 
 // Device-resident mutable state (one per system).
@@ -31,8 +32,10 @@ struct DevState {
 struct TbsmaParams {               // per type pair, pre-combined on the host
   // rho(r) = pre_rho exp(a_rho - b_rho r) S(r),  V(r) = pre_rep exp(a_rep - b_rep r) S(r)
   // fold != 0: ln(xi^2) and ln(2A) are folded into a_rho / a_rep and pre_* = 1 (all prefactors > 0)
-  double a_rho[kPairs], b_rho[kPairs], pre_rho[kPairs];
-  double a_rep[kPairs], b_rep[kPairs], pre_rep[kPairs];
+  // ak_* = a_* 64/ln2 and bk_* = b_* 64/ln2: the exponent in units of ln2/64, as exp_scaled() takes it
+  double ak_rho[kPairs], bk_rho[kPairs], b_rho[kPairs], pre_rho[kPairs];
+  double ak_rep[kPairs], bk_rep[kPairs], b_rep[kPairs], pre_rep[kPairs];
+  double m30_inv_w;                // -30 inv_w (dS/dr prefactor)
   double inv_w, t0;                // switch variable t = clamp(r inv_w + t0, 0, 1): inv_w = 1/(r_c - r_on), t0 = -r_on inv_w
   int fold;
 };
@@ -68,11 +71,12 @@ struct DevSys {
   // re-order scratch
   double4 *pos_tmp; double *vel_tmp; int *type_tmp, *orig_tmp;
   int *cell_id, *cell_count, *cell_start, *cell_fill, *perm, *scan_block;
-  // neighbour list, blocked ELL: entry k of the atom in (tile, lane) at nbr[(tile*cap + k)*32 + lane]
-  // entries that were inside r_c at build time are at k = 0 .. n_in-1, the others at k = cap-n_out .. cap-1;
-  // ncount = n_in | n_out << 16
+  // neighbour list, blocked ELL in groups of four: entries 4g .. 4g+3 of the atom in (tile, lane) are the 16 bytes at
+  // nbr[((tile*cap/4 + g)*32 + lane)*4] (cap is a multiple of 4), so a warp reads 512 contiguous bytes per group.
+  // Entries that were inside r_c at build time are at k = 0 .. n_in-1, the others at k = cap-n_out .. cap-1;
+  // the unused entries of a partly filled group are 0; ncount = n_in | n_out << 16
   unsigned *nbr; int *ncount;
-  const double *exp_tab;           // [64] 2^(j/64), correctly rounded (staged into shared memory by the passes)
+  const double *exp_tab;           // [kExpTabLen] 2^(j/64), correctly rounded (staged into shared memory by the passes), then LoopConsts
   // per-atom results
   double *rho, *eemb, *eatom;
   double *partial;                 // [n_blocks][8] block partial sums: E, Wxx,Wyy,Wzz,Wxy,Wxz,Wyz, (pad)
@@ -81,6 +85,10 @@ struct DevSys {
   TbsmaParams tb;
   TableParams tab;
 };
+
+// first entry of the list row of the atom in (tile, lane); entry k is at row[(k >> 2) * 128 + (k & 3)]
+__host__ __device__ inline size_t nbr_row_offset(size_t tile, int cap, int lane) { return (tile * (size_t)(cap >> 2) * 32 + lane) * 4; }
+__host__ __device__ inline size_t nbr_entry(int k) { return (size_t)(k >> 2) * 128 + (k & 3); }
 
 struct ProfClass { std::vector<cudaEvent_t> ev; size_t used = 0; long dropped = 0; };
 
@@ -95,6 +103,7 @@ struct md_system {
   bool opt_step_obs, opt_profile;
   int opt_force_variant;
   long steps, launches;
+  double exp_tab_host[md::kExpTabLen];
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
   int n_force_blocks;
   md::ProfClass prof[MD_K_COUNT];

@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   if (local >= s.npb) return;
   const int i = box * s.npb + local;
   const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
-  unsigned *row = s.nbr + tile * s.cap * 32 + (local & 31);
+  unsigned *row = s.nbr + nbr_row_offset(tile, s.cap, local & 31);
   const double4 pi = s.pos[i];
   const int cx = cell_coord(pi.x, s.cell_scale[0], s.nc[0]);
   const int cy = cell_coord(pi.y, s.cell_scale[1], s.nc[1]);
@@ -221,8 +221,8 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           if (r2 < s.rl2 && j != i) {
             const unsigned entry = (unsigned)j | ((kx | (ky << 2) | (kz << 4)) << kIdxBits);
             if (n_in + n_out < s.cap) {
-              if (r2 < s.rin2) row[(size_t)(n_in++) * 32] = entry;
-              else row[(size_t)(s.cap - 1 - n_out++) * 32] = entry;
+              if (r2 < s.rin2) row[nbr_entry(n_in++)] = entry;
+              else row[nbr_entry(s.cap - 1 - n_out++)] = entry;
             } else {
               overflow = true;
             }
@@ -233,6 +233,10 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     }
   }
   if (overflow) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
+  // the passes read whole groups of four: zero the unused entries of the two partly filled groups
+  const int first_out = s.cap - n_out;
+  for (int k = n_in; k < min((n_in + 3) & ~3, first_out); ++k) row[nbr_entry(k)] = 0u;
+  for (int k = max(first_out & ~3, n_in); k < first_out; ++k) row[nbr_entry(k)] = 0u;
   s.ncount[i] = n_in | (n_out << 16);
   // statistics: one atomic per warp
   const unsigned act = __activemask();
