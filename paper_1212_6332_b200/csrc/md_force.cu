@@ -20,9 +20,6 @@
 
 namespace md {
 
-#ifndef MD_PAIR2
-#define MD_PAIR2 1
-#endif
 #ifndef MD_FORCE_MINB
 #define MD_FORCE_MINB 5
 #endif
@@ -227,91 +224,93 @@ __device__ __forceinline__ void embed(const DevSys &s, int ti, double rho, doubl
 // ------------------------------------------------------------------------------------------------
 // list row walkers.  The row of the atom in (tile, lane) is a sequence of 16-byte groups of four entries, group g
 // at row[g * 32] (uint4 units).  Entries 0 .. n_in-1 were inside r_c at build time ("main"), entries cap-n_out ..
-// cap-1 were in the skin ("tail").  A walker keeps the entries of the next TWO groups and the gathered position of
-// the next pair in flight while a pair is evaluated: the list is a DRAM stream (latency ~1 us), the gathers hit L1/L2.
+// cap-1 were in the skin ("tail").
+//
+// Software pipeline.  prep(e, pj) turns a gathered neighbour into a PairD (d = x_j - x_i with its image, r2, w);
+// eval2 / eval1 run the potential on one or two PairDs.  While pairs k, k+1 are evaluated, the gathers of pairs k+2,
+// k+3 and the entries of the group after next are in flight.  ptxas gives every global load of the loop the SAME
+// scoreboard, and a scoreboard wait is a wait for ALL loads outstanding on it: a gather issued before the first use of
+// the previous gather would make that use wait for the new load's full latency (measured: 45 % of the stall samples).
+// So every load address carries `tok * zero`, where tok comes out of the preceding prep and zero is an integer that
+// is 0 at run time but not at compile time: the loads cannot be hoisted above the use of the data they would delay.
 // ------------------------------------------------------------------------------------------------
+struct PairD { double dx, dy, dz, r2, w; unsigned e; };
+
 __device__ __forceinline__ uint4 ldg_group(const uint4 *p) { return __ldg(p); }
 #define MD_GIDX(e) ((e) & kIdxMask)
 
-// One 256-bit load per gathered neighbour (LDG.E.256, sm_100): both passes are bound by the L1 data pipe, and a
-// 32-byte gather issued as two 128-bit loads costs twice the wavefronts.
+// One 256-bit load per gathered neighbour (LDG.E.256, sm_100) instead of two 128-bit loads.
 __device__ __forceinline__ double4 gather32(const double4 *p) {
   double4 v;
   asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
   return v;
 }
+__device__ __forceinline__ int order_token(const PairD &a) { return __double2loint(a.r2); }
 
-// body2 evaluates two pairs at once: their dependency chains are independent, which is what lets the FP64 pipe run near
-// its issue rate at the 4-5 resident warps per scheduler that the register budget allows (measured on B200: one
-// dependent DFMA chain per warp tops out at 64 % of the pipe, two at 77 %, four at 90 %).
-template <class Body2, class Body1>
-__device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, const double4 *__restrict__ pos, Body2 body2, Body1 body1) {
-  const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+// eval2 evaluates two pairs at once: their dependency chains are independent (measured on B200: one dependent DFMA
+// chain per warp tops out at 64 % of the FP64 pipe, two at 77 %, four at 90 %).
+template <class Prep, class Eval2, class Eval1>
+__device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, const double4 *__restrict__ pos, int zero, Prep prep,
+                                          Eval2 eval2, Eval1 eval1) {
+  const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2, nfull = n >> 2;
-  uint4 E = ng > 0 ? ldg_group(row) : zero;
-  uint4 En = ng > 1 ? ldg_group(row + 32) : zero;
+  uint4 E = ng > 0 ? ldg_group(row) : none;
+  uint4 En = ng > 1 ? ldg_group(row + 32) : none;
   double4 pA = gather32(pos + MD_GIDX(E.x));                      // slot 0 when there is no such pair: harmless
   double4 pB = gather32(pos + MD_GIDX(E.y));
-#if MD_PAIR2
   for (int g = 0; g < nfull; ++g) {
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : zero;
-    const double4 pC = gather32(pos + MD_GIDX(E.z));
-    const double4 pD = gather32(pos + MD_GIDX(E.w));
-    body2(E.x, pA, E.y, pB);
-    pA = gather32(pos + MD_GIDX(En.x));
-    pB = gather32(pos + MD_GIDX(En.y));
-    body2(E.z, pC, E.w, pD);
+    const PairD a = prep(E.x, pA), b = prep(E.y, pB);
+    const int t1 = (order_token(a) | order_token(b)) * zero;
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32 + t1) : none;
+    const double4 pC = gather32(pos + (MD_GIDX(E.z) + t1));
+    const double4 pD = gather32(pos + (MD_GIDX(E.w) + t1));
+    eval2(a, b);
+    const PairD c = prep(E.z, pC), d = prep(E.w, pD);
+    const int t2 = (order_token(c) | order_token(d)) * zero;
+    pA = gather32(pos + (MD_GIDX(En.x) + t2));
+    pB = gather32(pos + (MD_GIDX(En.y) + t2));
+    eval2(c, d);
     E = En; En = E2;
   }
   const int rem = n & 3;                                          // the partly filled last group
   if (rem >= 2) {
-    const double4 pC = gather32(pos + MD_GIDX(E.z));
-    body2(E.x, pA, E.y, pB);
-    if (rem == 3) body1(E.z, pC);
+    const PairD a = prep(E.x, pA), b = prep(E.y, pB);
+    const int t1 = (order_token(a) | order_token(b)) * zero;
+    const double4 pC = gather32(pos + (MD_GIDX(E.z) + t1));
+    eval2(a, b);
+    if (rem == 3) eval1(prep(E.z, pC));
   } else if (rem == 1) {
-    body1(E.x, pA);
+    eval1(prep(E.x, pA));
   }
-#else
-  for (int g = 0; g < nfull; ++g) {
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : zero;
-    const double4 pC = gather32(pos + MD_GIDX(E.z));
-    body1(E.x, pA);
-    const double4 pD = gather32(pos + MD_GIDX(E.w));
-    body1(E.y, pB);
-    pA = gather32(pos + MD_GIDX(En.x));
-    body1(E.z, pC);
-    pB = gather32(pos + MD_GIDX(En.y));
-    body1(E.w, pD);
-    E = En; En = E2;
-  }
-  const int rem = n & 3;
-  if (rem >= 1) body1(E.x, pA);
-  if (rem >= 2) body1(E.y, pB);
-  if (rem == 3) { const double4 pC = gather32(pos + MD_GIDX(E.z)); body1(E.z, pC); }
-#endif
 }
 
 // Tail: walked from the END of the row (entry cap-1-j, j = 0 .. n-1), so that every lane starts on a group boundary.
 // last = the last group of the row; mg = warp-uniform number of groups (max over the warp of ceil(n/4));
-// body(e, pj, active) is called by all 32 lanes.
-template <class Body>
-__device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n, int mg, const double4 *__restrict__ pos, Body body) {
-  const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+// body(PairD, active) is called by all 32 lanes.
+template <class Prep, class Body>
+__device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n, int mg, const double4 *__restrict__ pos, int zero, Prep prep,
+                                          Body body) {
+  const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2;
-  uint4 E = ng > 0 ? ldg_group(last) : zero;
-  uint4 En = ng > 1 ? ldg_group(last - 32) : zero;
+  uint4 E = ng > 0 ? ldg_group(last) : none;
+  uint4 En = ng > 1 ? ldg_group(last - 32) : none;
   double4 pA = gather32(pos + MD_GIDX(E.w));
+  double4 pB = gather32(pos + MD_GIDX(E.z));
   for (int g = 0; g < mg; ++g) {
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32) : zero;
     const int j = g * 4;
-    const double4 pB = gather32(pos + MD_GIDX(E.z));
-    body(E.w, pA, j < n);
-    const double4 pC = gather32(pos + MD_GIDX(E.y));
-    body(E.z, pB, j + 1 < n);
-    const double4 pD = gather32(pos + MD_GIDX(E.x));
-    body(E.y, pC, j + 2 < n);
-    pA = gather32(pos + MD_GIDX(En.w));
-    body(E.x, pD, j + 3 < n);
+    const PairD a = prep(E.w, pA), b = prep(E.z, pB);
+    const int t1 = (order_token(a) | order_token(b)) * zero;
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32 + t1) : none;
+    const double4 pC = gather32(pos + (MD_GIDX(E.y) + t1));
+    const double4 pD = gather32(pos + (MD_GIDX(E.x) + t1));
+    body(a, j < n);
+    body(b, j + 1 < n);
+    const PairD c = prep(E.y, pC), d = prep(E.x, pD);
+    const int t2 = (order_token(c) | order_token(d)) * zero;
+    pA = gather32(pos + (MD_GIDX(En.w) + t2));
+    pB = gather32(pos + (MD_GIDX(En.z) + t2));
+    body(c, j + 2 < n);
+    body(d, j + 3 < n);
     E = En; En = E2;
   }
 }
@@ -389,51 +388,45 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
 
   // main part: branch-free.  TB-SMA: the clamped switch makes a pair beyond r_c contribute exactly 0;
   // tables (no switch, reading A9): the strict test r2 < rc2 selects the term.
-  auto add1 = [&](double r2, int tp) {
-    const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, tp, r2);
-    if (KIND == MD_POT_TBSMA) rho += term;
-    else rho += (r2 < s.rc2) ? term : 0.0;
+  const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
+  auto prep = [&](unsigned e, const double4 &pj) {
+    PairD d;
+    d.r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, d.dx, d.dy, d.dz);
+    d.w = pj.w; d.e = e;
+    return d;
   };
-  walk_main(row.main, row.n_in, s.pos,
-            [&](unsigned eA, const double4 &pA, unsigned eB, const double4 &pB) {
-              double dx, dy, dz;
-              const double r2A = pair_r2<KIND != MD_POT_TBSMA>(pA, pi, eA, s, dx, dy, dz);
-              const double r2B = pair_r2<KIND != MD_POT_TBSMA>(pB, pi, eB, s, dx, dy, dz);
-              double tA, tB;
+  auto term1 = [&](const PairD &d) {
+    const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)d.w : 0, d.r2);
+    return (KIND == MD_POT_TBSMA || d.r2 < s.rc2) ? term : 0.0;
+  };
+  walk_main(row.main, row.n_in, s.pos, zero, prep,
+            [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
-                const double r2v[2] = {r2A, r2B};
+                const double r2v[2] = {a.r2, b.r2};
                 double tv[2];
                 density_term_n<FOLD, 2>(s, lc, tab, r2v, tv);
-                tA = tv[0]; tB = tv[1];
+                rho += tv[0]; rho2 += tv[1];
               } else {
-                tA = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pA.w : 0, r2A);
-                tB = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pB.w : 0, r2B);
+                rho += term1(a); rho2 += term1(b);
               }
-              if (KIND == MD_POT_TBSMA) { rho += tA; rho2 += tB; }
-              else { rho += (r2A < s.rc2) ? tA : 0.0; rho2 += (r2B < s.rc2) ? tB : 0.0; }
             },
-            [&](unsigned e, const double4 &pj) {
-              double dx, dy, dz;
-              const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
-              add1(r2, MULTI ? ti * s.nt + (int)pj.w : 0);
-            });
+            [&](const PairD &a) { rho += term1(a); });
   rho += rho2;
 
   // skin part: distance test only; a pair found inside r_c is parked (one slot per lane) and the warp evaluates
   // the parked pairs together when some lane needs its slot again, and once at the end
   const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
-  double park_r2 = 0.0; int park_tp = 0; bool parked = false;
-  walk_tail(row.last, row.n_out, mg, s.pos, [&](unsigned e, const double4 &pj, bool active) {
-    double dx, dy, dz;
-    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
-    const bool hit = active && r2 < s.rc2;
+  PairD park = {};
+  bool parked = false;
+  walk_tail(row.last, row.n_out, mg, s.pos, zero, prep, [&](const PairD &d, bool active) {
+    const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
-      if (parked) { rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, park_tp, park_r2); parked = false; }
+      if (parked) { rho += term1(park); parked = false; }
     }
-    if (hit) { park_r2 = r2; park_tp = MULTI ? ti * s.nt + (int)pj.w : 0; parked = true; }
+    if (hit) { park = d; parked = true; }
   });
   if (__any_sync(0xffffffffu, parked)) {
-    if (parked) rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, park_tp, park_r2);
+    if (parked) rho += term1(park);
   }
 
   if (!valid) return;
@@ -543,61 +536,49 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   const int ti = MULTI ? s.type[i] : 0;
   ForceAcc<OBS> acc, acc2;
 
-  walk_main(row.main, row.n_in, s.posf,
-            [&](unsigned eA, const double4 &pA, unsigned eB, const double4 &pB) {
-              double dxA, dyA, dzA, dxB, dyB, dzB, gA, gB, VA = 0.0, VB = 0.0;
-              const double r2A = pair_r2<KIND != MD_POT_TBSMA>(pA, pi, eA, s, dxA, dyA, dzA);
-              const double r2B = pair_r2<KIND != MD_POT_TBSMA>(pB, pi, eB, s, dxB, dyB, dzB);
+  const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
+  auto prep = [&](unsigned e, const double4 &pj) {
+    PairD d;
+    d.r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, d.dx, d.dy, d.dz);
+    d.w = pj.w; d.e = e;
+    return d;
+  };
+  auto eval1 = [&](const PairD &d, ForceAcc<OBS> &to) {
+    double g, V = 0.0;
+    const int tp = MULTI ? ti * s.nt + s.type[d.e & kIdxMask] : 0;
+    force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, d.r2, pi.w + d.w, g, V);
+    if (KIND != MD_POT_TBSMA && !(d.r2 < s.rc2)) { g = 0.0; V = 0.0; }   // tables: strict cut-off, no switch (reading A9)
+    force_accumulate<OBS>(to, g, V, d.dx, d.dy, d.dz);
+  };
+  walk_main(row.main, row.n_in, s.posf, zero, prep,
+            [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
-                const double r2v[2] = {r2A, r2B}, fpv[2] = {pi.w + pA.w, pi.w + pB.w};
+                const double r2v[2] = {a.r2, b.r2}, fpv[2] = {pi.w + a.w, pi.w + b.w};
                 double gv[2], Vv[2] = {0.0, 0.0};
                 force_term_n<OBS, FOLD, 2>(s, lc, tab, r2v, fpv, gv, Vv);
-                gA = gv[0]; gB = gv[1]; VA = Vv[0]; VB = Vv[1];
+                force_accumulate<OBS>(acc, gv[0], Vv[0], a.dx, a.dy, a.dz);
+                force_accumulate<OBS>(acc2, gv[1], Vv[1], b.dx, b.dy, b.dz);
               } else {
-                const int tpA = MULTI ? ti * s.nt + s.type[eA & kIdxMask] : 0, tpB = MULTI ? ti * s.nt + s.type[eB & kIdxMask] : 0;
-                force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tpA, r2A, pi.w + pA.w, gA, VA);
-                force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tpB, r2B, pi.w + pB.w, gB, VB);
+                eval1(a, acc); eval1(b, acc2);
               }
-              if (KIND != MD_POT_TBSMA) {                          // tables: strict cut-off, no switch (reading A9)
-                if (!(r2A < s.rc2)) { gA = 0.0; VA = 0.0; }
-                if (!(r2B < s.rc2)) { gB = 0.0; VB = 0.0; }
-              }
-              force_accumulate<OBS>(acc, gA, VA, dxA, dyA, dzA);
-              force_accumulate<OBS>(acc2, gB, VB, dxB, dyB, dzB);
             },
-            [&](unsigned e, const double4 &pj) {
-              double dx, dy, dz, g, V = 0.0;
-              const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
-              const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
-              force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, r2, pi.w + pj.w, g, V);
-              if (KIND != MD_POT_TBSMA && !(r2 < s.rc2)) { g = 0.0; V = 0.0; }
-              force_accumulate<OBS>(acc, g, V, dx, dy, dz);
-            });
+            [&](const PairD &a) { eval1(a, acc); });
   force_merge<OBS>(acc, acc2);
 
+  // skin part: distance test only; pairs found inside r_c are parked and evaluated together (see k_density)
   const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
-  double pk_dx = 0.0, pk_dy = 0.0, pk_dz = 0.0, pk_r2 = 1.0, pk_fp = 0.0; int pk_tp = 0; bool parked = false;
-  auto flush = [&]() {
-    double g, V = 0.0;
-    force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, pk_tp, pk_r2, pk_fp, g, V);
-    force_accumulate<OBS>(acc, g, V, pk_dx, pk_dy, pk_dz);
-    parked = false;
-  };
-  walk_tail(row.last, row.n_out, mg, s.posf, [&](unsigned e, const double4 &pj, bool active) {
-    double dx, dy, dz;
-    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
-    const bool hit = active && r2 < s.rc2;
+  PairD park = {};
+  park.r2 = 1.0;
+  bool parked = false;
+  walk_tail(row.last, row.n_out, mg, s.posf, zero, prep, [&](const PairD &d, bool active) {
+    const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
-      if (parked) flush();
+      if (parked) { eval1(park, acc); parked = false; }
     }
-    if (hit) {
-      pk_dx = dx; pk_dy = dy; pk_dz = dz; pk_r2 = r2; pk_fp = pi.w + pj.w;
-      pk_tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
-      parked = true;
-    }
+    if (hit) { park = d; parked = true; }
   });
   if (__any_sync(0xffffffffu, parked)) {
-    if (parked) flush();
+    if (parked) eval1(park, acc);
   }
 
   if (valid) {
