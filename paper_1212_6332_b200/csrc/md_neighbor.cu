@@ -180,6 +180,18 @@ __device__ __forceinline__ double min_image(double d, double L, double hL, unsig
   return d;
 }
 
+__device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-bit load on the read-only path
+  double4 v;
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
+}
+
+// PERCELL (every nc >= 5): two atoms of cells that are neighbours WITHOUT crossing the box boundary are closer than
+// 2L/nc <= 0.4 L per axis, and two atoms of cells that are neighbours ACROSS the boundary differ by more than 0.6 L, so
+// the branch of the canonical minimum image is decided by the pair of cells: the shift (0, -L or +L) and its image
+// code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
+// (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
+template <bool PERCELL>
 __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
@@ -199,40 +211,81 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   // pairs inside r_in (= r_c) now go to the front of the row (k = 0, 1, ...), skin pairs to the back (k = cap-1, cap-2, ...):
   // the two passes run the full pair evaluation only over the front part (md_force.cu)
   int n_in = 0, n_out = 0;
+  auto keep = [&](int j, double r2, unsigned code) {
+    const unsigned entry = (unsigned)j | (code << kIdxBits);
+    if (n_in + n_out < s.cap) {
+      if (r2 < s.rin2) row[nbr_entry(n_in++)] = entry;
+      else row[nbr_entry(s.cap - 1 - n_out++)] = entry;
+    } else {
+      overflow = true;
+    }
+    ++n_all;
+  };
+  // the same without branches (one predicated store), for the PERCELL candidate loop: almost every trip has SOME lane
+  // that accepts its candidate, so a branchy append runs for the whole warp on nearly every candidate
+  auto test_keep = [&](int j, double r2, unsigned code) {
+    const bool acc = r2 < s.rl2 && j != i;
+    const bool room = n_in + n_out < s.cap;
+    const bool in = r2 < s.rin2;
+    const int k = in ? n_in : s.cap - 1 - n_out;
+    if (acc && room) row[nbr_entry(k)] = (unsigned)j | (code << kIdxBits);
+    n_in += (acc && room && in) ? 1 : 0;
+    n_out += (acc && room && !in) ? 1 : 0;
+    n_all += acc ? 1 : 0;
+  };
   for (int ox = -1; ox <= 1; ++ox) {
-    int jx = cx + ox; jx += (jx < 0) ? ncx : 0; jx -= (jx >= ncx) ? ncx : 0;
+    int jx = cx + ox;
+    double sx = 0.0; unsigned kx = 0;
+    if (jx < 0) { jx += ncx; sx = -s.L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = s.L[0]; kx = 1; }
     for (int oy = -1; oy <= 1; ++oy) {
-      int jy = cy + oy; jy += (jy < 0) ? ncy : 0; jy -= (jy >= ncy) ? ncy : 0;
+      int jy = cy + oy;
+      double sy = 0.0; unsigned ky = 0;
+      if (jy < 0) { jy += ncy; sy = -s.L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = s.L[1]; ky = 1; }
       const int col = box * s.tnc + (jx * ncy + jy) * ncz;
       // up to three runs: the in-range z cells, plus the wrapped cell on either side
       for (int run = 0; run < 3; ++run) {
         int c0, c1;
+        double sz = 0.0; unsigned kz = 0;
         if (run == 0) { c0 = col + zlo; c1 = col + zhi; }
-        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; }
-        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; }
+        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; sz = -s.L[2]; kz = 2; }
+        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; sz = s.L[2]; kz = 1; }
         const int jbeg = s.cell_start[c0], jend = s.cell_start[c1 + 1];
-        for (int j = jbeg; j < jend; ++j) {
-          const double4 pj = s.pos[j];
-          unsigned kx, ky, kz;
-          const double dx = min_image(__dsub_rn(pj.x, pi.x), s.L[0], s.hL[0], kx);
-          const double dy = min_image(__dsub_rn(pj.y, pi.y), s.L[1], s.hL[1], ky);
-          const double dz = min_image(__dsub_rn(pj.z, pi.z), s.L[2], s.hL[2], kz);
-          const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-          if (r2 < s.rl2 && j != i) {
-            const unsigned entry = (unsigned)j | ((kx | (ky << 2) | (kz << 4)) << kIdxBits);
-            if (n_in + n_out < s.cap) {
-              if (r2 < s.rin2) row[nbr_entry(n_in++)] = entry;
-              else row[nbr_entry(s.cap - 1 - n_out++)] = entry;
-            } else {
-              overflow = true;
-            }
-            ++n_all;
+        if (PERCELL) {
+          // four candidates per trip: the four loads are issued together (read-only path, so the list stores
+          // in between cannot hold them back), then the four tests
+          const unsigned code = kx | (ky << 2) | (kz << 4);
+          auto dist2 = [&](const double4 &pj, double &r2) {
+            double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
+            if (code) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
+            r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          };
+          int j = jbeg;
+          for (; j + 4 <= jend; j += 4) {
+            const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
+            double r0, r1, r2, r3;
+            dist2(p0, r0); dist2(p1, r1); dist2(p2, r2); dist2(p3, r3);
+            test_keep(j, r0, code); test_keep(j + 1, r1, code); test_keep(j + 2, r2, code); test_keep(j + 3, r3, code);
+          }
+          for (; j < jend; ++j) {
+            double r2;
+            dist2(ld_pos(s.pos + j), r2);
+            test_keep(j, r2, code);
+          }
+        } else {
+          for (int j = jbeg; j < jend; ++j) {
+            const double4 pj = s.pos[j];
+            unsigned ax, ay, az;
+            const double dx = min_image(__dsub_rn(pj.x, pi.x), s.L[0], s.hL[0], ax);
+            const double dy = min_image(__dsub_rn(pj.y, pi.y), s.L[1], s.hL[1], ay);
+            const double dz = min_image(__dsub_rn(pj.z, pi.z), s.L[2], s.hL[2], az);
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (r2 < s.rl2 && j != i) keep(j, r2, ax | (ay << 2) | (az << 4));
           }
         }
       }
     }
   }
-  if (overflow) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
+  if (overflow || n_all > n_in + n_out) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
   // the passes read whole groups of four: zero the unused entries of the two partly filled groups
   const int first_out = s.cap - n_out;
   for (int k = n_in; k < min((n_in + 3) & ~3, first_out); ++k) row[nbr_entry(k)] = 0u;
@@ -285,7 +338,9 @@ int launch_rebuild_chain(md_system *sys) {
   }
   {
     ProfScope p(sys, MD_K_LIST);
-    ++sys->launches, k_build_list<<<d.nb * blocks_per_box(d.npb, kForceBlock), kForceBlock, 0, st>>>(d);
+    const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);
+    if (d.nc[0] >= 5 && d.nc[1] >= 5 && d.nc[2] >= 5) ++sys->launches, k_build_list<true><<<gl, kForceBlock, 0, st>>>(d);
+    else ++sys->launches, k_build_list<false><<<gl, kForceBlock, 0, st>>>(d);
     ++sys->launches, k_rebuild_end<<<1, 1, 0, st>>>(d);
   }
   return (int)cudaGetLastError();
