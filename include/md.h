@@ -149,8 +149,12 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                              (the paper's full-MD runs).  md_compute_forces always computes them.
  *  MD_OPT_PROFILE           1: bracket every kernel launch with CUDA events on the system's stream so that
  *                              md_profile_read can report per-kernel device time.
- *  MD_OPT_FORCE_VARIANT     0: choose by neighbour count; 1: thread-per-atom; 2: warp-per-atom. */
-enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3 };
+ *  MD_OPT_FORCE_VARIANT     0: choose by neighbour count; 1: thread-per-atom; 2: warp-per-atom.
+ *  MD_OPT_GRAPH             1 (default): md_step replays one CUDA graph per time step whose neighbour rebuild is
+ *                           the body of a conditional node (4 kernel launches per step when no rebuild is due);
+ *                           0: plain launches (every kernel of the rebuild chain is launched and returns at once
+ *                           unless a rebuild is due).  MD_OPT_PROFILE implies plain launches. */
+enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3, MD_OPT_GRAPH = 4 };
 int md_set_option(md_system *s, int option, int value);
 
 /* Kernel classes for md_profile_read */

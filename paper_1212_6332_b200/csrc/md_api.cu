@@ -5,6 +5,9 @@
 
 #include <new>
 
+#include <cstdio>
+#include <cstdlib>
+
 #include "md_internal.cuh"
 
 using namespace md;
@@ -78,7 +81,7 @@ static int geometry(const md_desc *d, Geometry &g) {
   if (g.cap > 0xfff0) return MD_EINVAL;               // ncount packs two 16-bit counts
   g.cap = (g.cap + 3) & ~3;
   g.tiles_per_box = (g.npb + 31) / 32;
-  g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock);
+  g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock / 8);   // block partials: enough for the 8-lanes-per-atom variant
   g.stage_bytes = (size_t)d->n_atoms * 3 * sizeof(double);
   if (g.stage_bytes < (1u << 20)) g.stage_bytes = 1u << 20;
   return MD_OK;
@@ -268,6 +271,86 @@ static int forces_sequence(md_system *s, bool observables, double half_dt) {
   return MD_OK;
 }
 
+static void drop_step_graph(md_system *s) {
+  if (s->step_exec) cudaGraphExecDestroy(s->step_exec);
+  if (s->step_graph) cudaGraphDestroy(s->step_graph);
+  s->step_exec = nullptr; s->step_graph = nullptr;
+}
+
+// One time step as a CUDA graph (built once per (dt, observables), replayed by md_step):
+//   k_kick_drift -> k_decide -> IF(do_rebuild){ clear, bin, 3 x scan, scatter, cell order, re-order, copy back, list } -> k_density -> k_force [-> k_reduce_boxes]
+// The rebuild decision stays on the device (k_decide sets the conditional node's handle), so md_step never
+// synchronises, and a step without a rebuild launches 4 kernels instead of 14.
+static int build_step_graph(md_system *s, double dt, bool obs) {
+  if (s->step_exec && s->step_dt == dt && s->step_obs == obs) return MD_OK;
+  drop_step_graph(s);
+  const long launches0 = s->launches;
+  // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot capture);
+  // nothing executes during capture, and the graph is launched on the caller's stream
+  cudaStream_t user = s->stream, st = nullptr;
+  if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); s->opt_graph = false; return MD_ECUDA; }
+  s->stream = st;
+  cudaGraph_t g = nullptr;
+  cudaGraphConditionalHandle cond;
+  bool ok = cudaGraphCreate(&g, 0) == cudaSuccess &&
+            cudaGraphConditionalHandleCreate(&cond, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+  const cudaGraphNode_t *deps = nullptr;
+  size_t ndeps = 0;
+  cudaGraphNode_t last = nullptr, cnode = nullptr;
+  cudaGraph_t tmp = nullptr;
+  long head = 0, body = 0, tail = 0;
+  if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    long l0 = s->launches;
+    ok = launch_kick_drift(s, dt) == 0 && launch_decide(s, cond, true) == 0;
+    head = s->launches - l0;
+    cudaStreamCaptureStatus cs;
+    if (ok) ok = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, &ndeps) == cudaSuccess && ndeps == 1;
+    if (ok) last = deps[0];
+    ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
+  }
+  if (ok) {
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = cond;
+    cp.conditional.type = cudaGraphCondTypeIf;
+    cp.conditional.size = 1;
+    ok = cudaGraphAddNode(&cnode, g, &last, 1, &cp) == cudaSuccess;
+    if (ok) {
+      cudaGraph_t bodyg = cp.conditional.phGraph_out[0];
+      ok = cudaStreamBeginCaptureToGraph(st, bodyg, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+      if (ok) {
+        long l0 = s->launches;
+        ok = launch_rebuild_body(s) == 0;
+        body = s->launches - l0;
+        ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
+      }
+    }
+  }
+  if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, &cnode, nullptr, 1, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    long l0 = s->launches;
+    ok = launch_density(s) == 0 && launch_force(s, obs, 0.5 * dt) == 0;
+    tail = s->launches - l0;
+    ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
+  }
+  cudaGraphExec_t exec = nullptr;
+  if (ok) ok = cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
+  s->launches = launches0;
+  s->stream = user;
+  cudaStreamDestroy(st);
+  if (!ok) {
+    const cudaError_t err = cudaGetLastError();      // fall back to plain launches (e.g. a driver without conditional nodes)
+    if (getenv("MD_DEBUG")) fprintf(stderr, "md: step graph unavailable (%s; head %ld body %ld tail %ld, deps %zu)\n", cudaGetErrorString(err), head, body, tail, ndeps);
+    if (g) cudaGraphDestroy(g);
+    s->opt_graph = false;
+    return MD_ECUDA;
+  }
+  s->step_graph = g; s->step_exec = exec; s->step_dt = dt; s->step_obs = obs;
+  s->step_kernels = (int)(head + tail); s->body_kernels = (int)body;
+  return MD_OK;
+}
+
 static int request_rebuild(md_system *s) {
   const int one = 1;
   return check_cuda(cudaMemcpyAsync(&s->d.st->force_rebuild, &one, sizeof(int), cudaMemcpyHostToDevice, s->stream));
@@ -327,7 +410,8 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->stream = (cudaStream_t)d->stream;
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
-  s->opt_step_obs = s->opt_profile = false; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
+  s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
+  s->step_graph = nullptr; s->step_exec = nullptr; s->step_dt = 0.0; s->step_obs = false; s->step_kernels = s->body_kernels = 0;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
   o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
@@ -418,6 +502,7 @@ int md_destroy(md_system *s) {
   if (!s) return MD_OK;
   cudaStreamSynchronize(s->stream);
   for (auto &p : s->prof) for (cudaEvent_t ev : p.ev) cudaEventDestroy(ev);
+  drop_step_graph(s);
   delete s;
   return MD_OK;
 }
@@ -427,7 +512,8 @@ int md_set_option(md_system *s, int option, int value) {
   switch (option) {
     case MD_OPT_STEP_OBSERVABLES: s->opt_step_obs = value != 0; return MD_OK;
     case MD_OPT_PROFILE: s->opt_profile = value != 0; return MD_OK;
-    case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; return MD_OK;
+    case MD_OPT_GRAPH: s->opt_graph = value != 0; return MD_OK;
+    case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
   }
   return MD_EINVAL;
 }
@@ -479,9 +565,17 @@ int md_step(md_system *s, int n, double dt) {
   if (n == 0) return MD_OK;
   if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
   if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
-  for (int k = 0; k < n; ++k) {
-    if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
-    if ((rc = forces_sequence(s, s->opt_step_obs, 0.5 * dt)) != MD_OK) return rc;
+  if (s->opt_graph && !s->opt_profile && build_step_graph(s, dt, s->opt_step_obs) == MD_OK) {
+    // one graph launch per step: 4 kernels when no rebuild is due, no launch of the chain's kernels at all
+    for (int k = 0; k < n; ++k)
+      if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) return MD_ECUDA;
+    s->launches += (long)n * s->step_kernels;
+    s->have_list = true; s->forces_valid = true; s->observables_valid = s->opt_step_obs;
+  } else {
+    for (int k = 0; k < n; ++k) {
+      if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
+      if ((rc = forces_sequence(s, s->opt_step_obs, 0.5 * dt)) != MD_OK) return rc;
+    }
   }
   s->steps += n;
   return MD_OK;
@@ -614,7 +708,7 @@ int md_get_stats(md_system *s, md_stats *out) {
   if (cudaMemcpyAsync(&st, s->d.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
   if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   out->steps = s->steps; out->rebuilds = (long)st.rebuilds; out->max_neighbors = st.max_neighbors;
-  out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap; out->kernel_launches = s->launches; out->list_entries = (long)st.list_entries;
+  out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap; out->kernel_launches = s->launches + (long)st.graph_body_runs * s->body_kernels; out->list_entries = (long)st.list_entries;
   return MD_OK;
 }
 

@@ -520,6 +520,45 @@ __device__ __forceinline__ void force_merge(ForceAcc<OBS> &a, const ForceAcc<OBS
   if constexpr (OBS) { a.ev += b.ev; a.w0 += b.w0; a.w1 += b.w1; a.w2 += b.w2; a.w3 += b.w3; a.w4 += b.w4; a.w5 += b.w5; }
 }
 
+// Epilogue of the force pass for the thread that holds the totals of atom i (valid) or nothing (!valid): store the
+// force, second half-kick, non-finite flag; OBS: per-atom energy and the block's partial sums of E and W.
+template <bool OBS>
+__device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &kick, int i, bool valid, int ti, const ForceAcc<OBS> &acc,
+                                             double (*sm)[8]) {
+  if (valid) {
+    const size_t N = (size_t)s.N;
+    s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
+    const double h = kick.h[ti];
+    if (h != 0.0) { s.vel[i] += h * acc.fx; s.vel[N + i] += h * acc.fy; s.vel[2 * N + i] += h * acc.fz; }
+    if (!(fabs(acc.fx) + fabs(acc.fy) + fabs(acc.fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
+  }
+  if constexpr (OBS) {
+    double e_i = 0.0;
+    if (valid) { e_i = s.eemb[i] + 0.5 * acc.ev; s.eatom[i] = e_i; }
+    // warp-shuffle reduction (fixed butterfly order => deterministic), then across the 4 warps
+    double v[7] = {e_i, 0.5 * acc.w0, 0.5 * acc.w1, 0.5 * acc.w2, 0.5 * acc.w3, 0.5 * acc.w4, 0.5 * acc.w5};
+    if (!valid) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) v[c] = 0.0;
+    }
+#pragma unroll
+    for (int c = 0; c < 7; ++c)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0)
+#pragma unroll
+      for (int c = 0; c < 7; ++c) sm[wid][c] = v[c];
+    __syncthreads();
+    if (threadIdx.x < 7) {
+      double a = 0.0;
+#pragma unroll
+      for (int w = 0; w < kForceBlock / 32; ++w) a += sm[w][threadIdx.x];
+      s.partial[(size_t)blockIdx.x * 8 + threadIdx.x] = a;
+    }
+  }
+}
+
 template <int KIND, bool MULTI, bool OBS, bool FOLD>
 __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
   __shared__ double tab_sm[kExpTabLen];
@@ -581,38 +620,112 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     if (parked) eval1(park, acc);
   }
 
-  if (valid) {
-    const size_t N = (size_t)s.N;
-    s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
-    const double h = kick.h[ti];
-    if (h != 0.0) { s.vel[i] += h * acc.fx; s.vel[N + i] += h * acc.fy; s.vel[2 * N + i] += h * acc.fz; }
-    if (!(fabs(acc.fx) + fabs(acc.fy) + fabs(acc.fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
+  force_finish<OBS>(s, kick, i, valid, ti, acc, sm);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small systems: kSub lanes per atom.  With one thread per atom a system of a few thousand atoms fills a fraction of
+// the SMs and every thread walks its ~50 pairs one after the other (tens of microseconds of pure latency).  Here the
+// kSub lanes of an atom take the 16-byte groups of its row round-robin and their partial sums are combined by
+// shuffles in a fixed order (deterministic).  Same arithmetic per pair as the kernels above.
+// ------------------------------------------------------------------------------------------------
+constexpr int kSub = 8, kSubAtoms = kForceBlock / kSub;
+
+struct SubMap { int box, local, i, sl; bool valid; };
+__device__ __forceinline__ SubMap sub_map(const DevSys &s) {
+  SubMap m;
+  const int bpb = (s.npb + kSubAtoms - 1) / kSubAtoms;
+  m.box = blockIdx.x / bpb;
+  m.local = (blockIdx.x - m.box * bpb) * kSubAtoms + (threadIdx.x / kSub);
+  m.sl = threadIdx.x % kSub;
+  m.valid = m.local < s.npb;
+  m.i = m.box * s.npb + (m.valid ? m.local : 0);
+  return m;
+}
+
+// calls body(entry, in_main) for the entries of the row that this sub-lane owns
+template <class Body>
+__device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, Body body) {
+  for (int g = sl; g * 4 < row.n_in; g += kSub) {
+    const uint4 E = ldg_group(row.main + (size_t)g * 32);
+    const unsigned e[4] = {E.x, E.y, E.z, E.w};
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      if (g * 4 + c < row.n_in) body(e[c], true);
   }
-  if constexpr (OBS) {
-    double e_i = 0.0;
-    if (valid) { e_i = s.eemb[i] + 0.5 * acc.ev; s.eatom[i] = e_i; }
-    // warp-shuffle reduction (fixed butterfly order => deterministic), then across the 4 warps
-    double v[7] = {e_i, 0.5 * acc.w0, 0.5 * acc.w1, 0.5 * acc.w2, 0.5 * acc.w3, 0.5 * acc.w4, 0.5 * acc.w5};
-    if (!valid) {
+  for (int g = sl; g * 4 < row.n_out; g += kSub) {
+    const uint4 E = ldg_group(row.last - (size_t)g * 32);
+    const unsigned e[4] = {E.w, E.z, E.y, E.x};
 #pragma unroll
-      for (int c = 0; c < 7; ++c) v[c] = 0.0;
+    for (int c = 0; c < 4; ++c)
+      if (g * 4 + c < row.n_out) body(e[c], false);
+  }
+}
+
+template <int KIND, bool MULTI, bool FOLD>
+__global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_constant__ DevSys s) {
+  __shared__ double tab_sm[kExpTabLen];
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
+  const SubMap m = sub_map(s);
+  const AtomRow row = atom_row(s, m.box, m.local, m.i, m.valid);
+  const double4 pi = s.pos[m.i];
+  const int ti = MULTI ? (int)pi.w : 0;
+  double rho = 0.0;
+  walk_sub(row, m.sl, [&](unsigned e, bool in_main) {
+    const double4 pj = gather32(s.pos + MD_GIDX(e));
+    double dx, dy, dz;
+    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
+    // main: TB-SMA is switched off continuously beyond r_c, tables need the strict test; skin: only pairs now inside r_c
+    if ((in_main && KIND == MD_POT_TBSMA) || r2 < s.rc2)
+      rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pj.w : 0, r2);
+  });
+#pragma unroll
+  for (int o = 1; o < kSub; o <<= 1) rho += __shfl_xor_sync(0xffffffffu, rho, o);
+  if (!m.valid || m.sl != 0) return;
+  double F, Fp;
+  embed<KIND>(s, ti, rho, F, Fp);
+  if (!(fabs(Fp) <= 1.79e308) || !(fabs(rho) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
+  s.rho[m.i] = rho;
+  s.eemb[m.i] = F;
+  s.posf[m.i] = make_double4(pi.x, pi.y, pi.z, Fp);
+}
+
+template <int KIND, bool MULTI, bool OBS, bool FOLD>
+__global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant__ DevSys s, const KickParams kick) {
+  __shared__ double tab_sm[kExpTabLen];
+  __shared__ double sm[kForceBlock / 32][8];
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
+  const SubMap m = sub_map(s);
+  const AtomRow row = atom_row(s, m.box, m.local, m.i, m.valid);
+  const double4 pi = s.posf[m.i];
+  const int ti = MULTI ? s.type[m.i] : 0;
+  ForceAcc<OBS> acc;
+  walk_sub(row, m.sl, [&](unsigned e, bool in_main) {
+    const double4 pj = gather32(s.posf + MD_GIDX(e));
+    double dx, dy, dz, g, V = 0.0;
+    const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
+    if ((in_main && KIND == MD_POT_TBSMA) || r2 < s.rc2) {
+      const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
+      force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, r2, pi.w + pj.w, g, V);
+      force_accumulate<OBS>(acc, g, V, dx, dy, dz);
     }
+  });
 #pragma unroll
-    for (int c = 0; c < 7; ++c)
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (lane == 0)
-#pragma unroll
-      for (int c = 0; c < 7; ++c) sm[wid][c] = v[c];
-    __syncthreads();
-    if (threadIdx.x < 7) {
-      double a = 0.0;
-#pragma unroll
-      for (int w = 0; w < kForceBlock / 32; ++w) a += sm[w][threadIdx.x];
-      s.partial[(size_t)blockIdx.x * 8 + threadIdx.x] = a;
+  for (int o = 1; o < kSub; o <<= 1) {
+    acc.fx += __shfl_xor_sync(0xffffffffu, acc.fx, o); acc.fy += __shfl_xor_sync(0xffffffffu, acc.fy, o);
+    acc.fz += __shfl_xor_sync(0xffffffffu, acc.fz, o);
+    if constexpr (OBS) {
+      acc.ev += __shfl_xor_sync(0xffffffffu, acc.ev, o);
+      acc.w0 += __shfl_xor_sync(0xffffffffu, acc.w0, o); acc.w1 += __shfl_xor_sync(0xffffffffu, acc.w1, o);
+      acc.w2 += __shfl_xor_sync(0xffffffffu, acc.w2, o); acc.w3 += __shfl_xor_sync(0xffffffffu, acc.w3, o);
+      acc.w4 += __shfl_xor_sync(0xffffffffu, acc.w4, o); acc.w5 += __shfl_xor_sync(0xffffffffu, acc.w5, o);
     }
   }
+  force_finish<OBS>(s, kick, m.i, m.valid && m.sl == 0, ti, acc, sm);
 }
 
 // per box: sum the block partials in a fixed order
@@ -672,15 +785,30 @@ int launch_prepare_tables(md_system *sys) {
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
+// variant of the two passes: kSub lanes per atom while one thread per atom would leave SMs idle
+bool use_sub_lanes(const md_system *sys) {
+  if (sys->opt_force_variant == 1) return false;
+  if (sys->opt_force_variant == 2) return true;
+  return sys->d.N <= kSubMaxAtoms;
+}
+int force_blocks(const md_system *sys) {
+  return sys->d.nb * blocks_per_box(sys->d.npb, use_sub_lanes(sys) ? kSubAtoms : kForceBlock);
+}
+
 template <int KIND, bool FOLD>
 static void launch_density_k(md_system *sys, int grid) {
+  if (use_sub_lanes(sys)) {
+    if (sys->d.nt > 1) ++sys->launches, k_density_sub<KIND, true, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    else ++sys->launches, k_density_sub<KIND, false, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    return;
+  }
   if (sys->d.nt > 1) ++sys->launches, k_density<KIND, true, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
   else ++sys->launches, k_density<KIND, false, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
 }
 
 int launch_density(md_system *sys) {
   ProfScope p(sys, MD_K_DENSITY);
-  const int grid = sys->d.nb * blocks_per_box(sys->d.npb, kForceBlock);
+  const int grid = force_blocks(sys);
   if (sys->d.kind == MD_POT_TBSMA) {
     if (sys->d.tb.fold) launch_density_k<MD_POT_TBSMA, true>(sys, grid);
     else launch_density_k<MD_POT_TBSMA, false>(sys, grid);
@@ -693,6 +821,16 @@ static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams 
   const bool multi = sys->d.nt > 1;
   cudaStream_t st = sys->stream;
   ++sys->launches;
+  if (use_sub_lanes(sys)) {
+    if (multi) {
+      if (obs) k_force_sub<KIND, true, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force_sub<KIND, true, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    } else {
+      if (obs) k_force_sub<KIND, false, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force_sub<KIND, false, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    }
+    return;
+  }
   if (multi) {
     if (obs) k_force<KIND, true, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
     else k_force<KIND, true, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
@@ -705,7 +843,7 @@ static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams 
 int launch_force(md_system *sys, bool observables, double half_dt) {
   KickParams kp;
   for (int t = 0; t < MD_MAX_TYPES; ++t) kp.h[t] = (t < sys->d.nt) ? half_dt / sys->mass_ev[t] : 0.0;
-  const int grid = sys->d.nb * blocks_per_box(sys->d.npb, kForceBlock);
+  const int grid = force_blocks(sys);
   {
     ProfScope p(sys, MD_K_FORCE);
     if (sys->d.kind == MD_POT_TBSMA) {
@@ -715,7 +853,7 @@ int launch_force(md_system *sys, bool observables, double half_dt) {
   }
   if (observables) {
     ProfScope p(sys, MD_K_REDUCE);
-    ++sys->launches, k_reduce_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, blocks_per_box(sys->d.npb, kForceBlock));
+    ++sys->launches, k_reduce_boxes<<<sys->d.nb, 256, 0, sys->stream>>>(sys->d, force_blocks(sys) / sys->d.nb);
   }
   return (int)cudaGetLastError();
 }

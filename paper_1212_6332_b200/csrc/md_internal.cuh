@@ -27,6 +27,7 @@ struct DevState {
   int max_neighbors;               // of the last build
   unsigned long long rebuilds;
   unsigned long long list_entries; // sum of list lengths of the last build
+  unsigned long long graph_body_runs; // rebuild bodies that ran inside a CUDA-graph step (for the launch count)
 };
 
 struct TbsmaParams {               // per type pair, pre-combined on the host
@@ -100,7 +101,9 @@ struct md_system {
   double mass_ev[MD_MAX_TYPES];    // eV fs^2 / A^2
   double cutoff, skin;
   bool have_list, forces_valid, observables_valid;
-  bool opt_step_obs, opt_profile;
+  bool opt_step_obs, opt_profile, opt_graph;
+  // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
+  cudaGraph_t step_graph; cudaGraphExec_t step_exec; double step_dt; bool step_obs; int step_kernels, body_kernels;
   int opt_force_variant;
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];
@@ -112,10 +115,15 @@ struct md_system {
 namespace md {
 // launch geometry of the per-atom kernels that use the tile mapping
 constexpr int kForceBlock = 128;
+constexpr int kSubMaxAtoms = 24576;                // at or below this many atoms the passes use 8 lanes per atom (md_force.cu)
+bool use_sub_lanes(const md_system *s);
+int force_blocks(const md_system *s);              // grid of the two passes (and number of block partials)
 inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block; }
 
 // launchers (each enqueues on s->stream; returns cudaError_t of the launch)
-int launch_rebuild_chain(md_system *s);                       // conditional on DevState (force_rebuild / maxd2)
+int launch_rebuild_chain(md_system *s);                       // decision + body, conditional on DevState (force_rebuild / maxd2)
+int launch_decide(md_system *s, cudaGraphConditionalHandle cond, bool use_cond);
+int launch_rebuild_body(md_system *s);
 int launch_density(md_system *s);
 int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
 int launch_force(md_system *s, bool observables, double half_dt); // half_dt = dt/2 (0: no velocity update)

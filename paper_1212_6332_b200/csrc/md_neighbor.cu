@@ -20,18 +20,25 @@ __device__ __forceinline__ int cell_coord(double x, double scale, int nc) {
   return max(0, min(c, nc - 1));
 }
 
-// ---- K0: decision + clear the cell counters ---------------------------------------------------
-__global__ void k_rebuild_begin(const __grid_constant__ DevSys s, unsigned long long thr2_bits) {
-  const DevState *st = s.st;
+// ---- K0: decision (one thread), then clear the cell counters -------------------------------------
+// The decision is taken on the device: rebuild if the host asked for it or if the largest displacement since the
+// last build exceeds skin/2 (strict >, reading A11).  When md_step runs as a CUDA graph, the rest of the chain sits
+// in the body of a conditional IF node and `cond` is its handle; otherwise every kernel of the chain is launched
+// and returns at once unless do_rebuild is set.
+__global__ void k_decide(const __grid_constant__ DevSys s, unsigned long long thr2_bits, cudaGraphConditionalHandle cond, int use_cond) {
+  DevState *st = s.st;
   const bool go = st->force_rebuild != 0 || st->maxd2_bits > thr2_bits;
-  const int gid = blockIdx.x * blockDim.x + threadIdx.x;
-  if (go)
-    for (int c = gid; c <= s.ncell; c += gridDim.x * blockDim.x) { s.cell_count[c] = 0; s.cell_fill[c] = 0; }
-  if (gid == 0) {
-    s.st->do_rebuild = go ? 1 : 0;
-    s.st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
-    if (go) { s.st->max_neighbors = 0; s.st->list_entries = 0ull; }
-  }
+  st->do_rebuild = go ? 1 : 0;
+  st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
+  st->maxd2_bits = 0ull;
+  st->force_rebuild = 0;
+  if (go) { st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1; }
+  if (use_cond) { cudaGraphSetConditional(cond, go ? 1u : 0u); if (go) st->graph_body_runs += 1; }
+}
+
+__global__ void k_clear_cells(const __grid_constant__ DevSys s) {
+  if (!s.st->do_rebuild) return;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= s.ncell; c += gridDim.x * blockDim.x) { s.cell_count[c] = 0; s.cell_fill[c] = 0; }
 }
 
 // ---- K1: wrap, cell index (paper's dIC, G1-G3), histogram (paper's hNAC) ---------------------
@@ -300,24 +307,24 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   }
 }
 
-// ---- K10: close the chain ---------------------------------------------------------------------------
-__global__ void k_rebuild_end(const __grid_constant__ DevSys s) {
-  DevState *st = s.st;
-  if (st->do_rebuild) st->rebuilds += 1;
-  st->maxd2_bits = 0ull;
-  st->force_rebuild = 0;
+int launch_decide(md_system *sys, cudaGraphConditionalHandle cond, bool use_cond) {
+  const DevSys &d = sys->d;
+  const unsigned long long thr_bits = (unsigned long long)__builtin_bit_cast(long long, d.thr2);
+  ProfScope p(sys, MD_K_BIN);
+  ++sys->launches, k_decide<<<1, 1, 0, sys->stream>>>(d, thr_bits, cond, use_cond ? 1 : 0);
+  return (int)cudaGetLastError();
 }
 
-int launch_rebuild_chain(md_system *sys) {
+// wrap, bin, scan, scatter, per-cell order, re-order, list: every kernel returns at once unless do_rebuild is set
+int launch_rebuild_body(md_system *sys) {
   const DevSys &d = sys->d;
   cudaStream_t st = sys->stream;
   const int N = d.N, tb = 256, gN = (N + tb - 1) / tb;
-  const unsigned long long thr_bits = (unsigned long long)__builtin_bit_cast(long long, d.thr2);
   const int nscan = (d.ncell + 1 + kScanTile - 1) / kScanTile;
   {
     ProfScope p(sys, MD_K_BIN);
     int g0 = (d.ncell + 1 + tb - 1) / tb; if (g0 > 1184) g0 = 1184;
-    ++sys->launches, k_rebuild_begin<<<g0, tb, 0, st>>>(d, thr_bits);
+    ++sys->launches, k_clear_cells<<<g0, tb, 0, st>>>(d);
     ++sys->launches, k_bin<<<gN, tb, 0, st>>>(d);
   }
   {
@@ -341,9 +348,15 @@ int launch_rebuild_chain(md_system *sys) {
     const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);
     if (d.nc[0] >= 5 && d.nc[1] >= 5 && d.nc[2] >= 5) ++sys->launches, k_build_list<true><<<gl, kForceBlock, 0, st>>>(d);
     else ++sys->launches, k_build_list<false><<<gl, kForceBlock, 0, st>>>(d);
-    ++sys->launches, k_rebuild_end<<<1, 1, 0, st>>>(d);
   }
   return (int)cudaGetLastError();
+}
+
+int launch_rebuild_chain(md_system *sys) {
+  cudaGraphConditionalHandle none{};
+  int rc = launch_decide(sys, none, false);
+  if (rc != 0) return rc;
+  return launch_rebuild_body(sys);
 }
 
 }  // namespace md

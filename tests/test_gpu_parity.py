@@ -127,6 +127,49 @@ def test_step_with_observables_matches_plain_step(md):
     assert np.abs(a.positions() - b.positions()).max() < 1e-11 and np.abs(a.velocities() - b.velocities()).max() < 1e-12
 
 
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small"])
+def test_both_pass_variants(md, case, variant):
+    """One thread per atom (what large systems run) and 8 lanes per atom (small systems), forced on the same input."""
+    w = CASES[case]()
+    o = oracle_of(w)
+    of, oe, ow = o.compute_forces()
+    orho, ofp = o.densities()
+    g = md.MDSystem(w)
+    g.set_option(md.MD_OPT_FORCE_VARIANT, variant)
+    gf, ge, gw = g.compute_forces()
+    grho, gfp = g.densities()
+    assert np.abs(grho - orho).max() <= 1e-12 * np.abs(orho).max()
+    assert np.abs(gfp - ofp).max() <= 1e-12 * np.abs(ofp).max()
+    assert np.abs(gf - of).max() <= F_TOL
+    assert np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    assert np.abs(gw - ow).max() <= 1e-11 * np.abs(ow).max()
+    o.step(30, w.dt)
+    g.step(30, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+
+
+@pytest.mark.parametrize("case", ["cfg0", "cfg2_small", "cfg4_small"])
+def test_graph_step_equals_plain_launches(md, case):
+    """md_step as a CUDA graph with the rebuild in a conditional node runs the same kernels as the plain launches."""
+    w = CASES[case]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    b.set_option(md.MD_OPT_GRAPH, 0)
+    for n in (1, 7, 40):
+        a.step(n, w.dt)
+        b.step(n, w.dt)
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    sa, sb = a.stats(), b.stats()
+    assert sa["rebuilds"] == sb["rebuilds"] and sa["rebuilds"] >= 2 and sa["error_flags"] == 0
+    assert sa["kernel_launches"] < sb["kernel_launches"]          # the chain is launched only when a rebuild is due
+    # a different dt re-builds the graph
+    a.step(5, 0.5 * w.dt)
+    b.step(5, 0.5 * w.dt)
+    assert np.array_equal(a.positions(), b.positions())
+
+
 def test_run_to_run_determinism(md):
     w = CASES["cfg2_small"]()
     res = []
