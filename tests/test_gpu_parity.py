@@ -34,6 +34,10 @@ CASES = {
     "cfg3b_small": lambda: workloads.config("3b", scale=12),               # 6.5 A cut-off, ~134 list entries
     "cfg4_small": lambda: workloads.config(4, scale=12),                   # W tables + PKA
     "noncubic": lambda: _noncubic(),
+    # binary alloys: every type-pair parameter set / table differs, two masses
+    "alloy_tbsma": lambda: workloads.alloy(workloads.config("3a", scale=10), 21),           # 4000 atoms
+    "alloy_tbsma_boxes": lambda: workloads.alloy(workloads.config(2, scale=5), 22, 0.3),    # 5 boxes x 500, 30 % type 1
+    "alloy_tables": lambda: workloads.alloy(workloads.config(1, scale=10), 23),             # 2000 atoms, 4 pair tables
 }
 
 
@@ -89,7 +93,8 @@ def test_density_force_energy_virial(md, case):
 
 
 @pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 100), ("cfg1_small", 100), ("cfg2_small", 100),
-                                         ("cfg3b_small", 40), ("cfg4_small", 100)])
+                                         ("cfg3b_small", 40), ("cfg4_small", 100), ("alloy_tbsma", 100),
+                                         ("alloy_tbsma_boxes", 60), ("alloy_tables", 100)])
 def test_trajectory(md, case, nsteps):
     w = CASES[case]()
     o = oracle_of(w)
@@ -128,7 +133,8 @@ def test_step_with_observables_matches_plain_step(md):
 
 
 @pytest.mark.parametrize("variant", [1, 2])
-@pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small"])
+@pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small", "alloy_tbsma",
+                                  "alloy_tables"])
 def test_both_pass_variants(md, case, variant):
     """One thread per atom (what large systems run) and 8 lanes per atom (small systems), forced on the same input."""
     w = CASES[case]()

@@ -433,3 +433,87 @@ def test_isolated_atom_and_empty_neighbourhood():
     f, e, vir = o.compute_forces()
     assert np.all(f == 0) and np.all(e == 0) and np.all(vir == 0)
     assert np.all(o.neighbors()[0] == 0)
+
+
+# ---------------------------------------------------------------- binary alloys (PAPER.md:78 rho^(ab), V^(ab))
+def _alloy_energy_numpy(pos, types, tb, cutoff):
+    """eq.(1) with type-pair parameters written out in numpy (direct double loop, float64); index [ti*2 + tj]."""
+    ron = tb["taper_on"]
+    etot, n = 0.0, len(pos)
+    for i in range(n):
+        rho = pair = 0.0
+        for j in range(n):
+            if i == j:
+                continue
+            r = float(np.sqrt(((pos[i] - pos[j]) ** 2).sum()))
+            if r >= cutoff:
+                continue
+            k = types[i] * 2 + types[j]
+            t = min(max((r - ron) / (cutoff - ron), 0.0), 1.0)
+            s = 1.0 - t ** 3 * (10.0 - 15.0 * t + 6.0 * t * t)
+            x = r / tb["r0"][k] - 1.0
+            rho += tb["xi"][k] ** 2 * np.exp(-2.0 * tb["q"][k] * x) * s
+            pair += 2.0 * tb["A"][k] * np.exp(-tb["p"][k] * x) * s
+        etot += -np.sqrt(rho) + 0.5 * pair
+    return etot
+
+
+def test_alloy_energy_and_forces_against_numpy_definition():
+    """type-pair indexing of every parameter: energy from the definition, forces from its central differences."""
+    w = workloads.alloy(workloads.config(0, scale=5), 11)
+    rng = np.random.default_rng(3)
+    idx = rng.choice(w.n_atoms, 24, replace=False)
+    pos = w.positions[idx] * 0.55 + 20.0                # a dense random cluster in a big box, both types present
+    types = w.types[idx]
+    assert 4 < types.sum() < 20
+    kw = dict(pot_kind=0, mass=w.mass, tbsma=w.tbsma, box=np.full(3, 60.0), cutoff=4.9, skin=0.3,
+              velocities=np.zeros((24, 3)), types=types, n_boxes=1)
+    f, e, _ = Oracle(positions=pos, **kw).compute_forces()
+    eref = _alloy_energy_numpy(pos, types, w.tbsma, 4.9)
+    assert abs(e.sum() - eref) < 1e-12 * abs(eref)
+    h = 1e-4
+    for a, c in ((0, 0), (5, 1), (17, 2)):
+        def E(dh):
+            p2 = pos.copy(); p2[a, c] += dh
+            return _alloy_energy_numpy(p2, types, w.tbsma, 4.9)
+        fd = -((8 * (E(h) - E(-h)) - (E(2 * h) - E(-2 * h))) / (12 * h))
+        assert abs(fd - f[a, c]) < 2e-8 * max(1.0, abs(f[a, c]))
+
+
+@pytest.mark.parametrize("cfg", ["0", "1"])
+def test_alloy_reduces_to_one_species_and_label_swap(cfg):
+    base = workloads.config(cfg, scale=5 if cfg == "0" else 7)
+    w = workloads.alloy(base, 5)
+    # (a) identical parameter sets for every pair == the one-species system, whatever the labels
+    same = workloads.Workload(**{**w.__dict__})
+    if cfg == "0":
+        same.tbsma = {k: (np.repeat(base.tbsma[k], 4) if k != "taper_on" else base.tbsma[k]) for k in base.tbsma}
+    else:
+        t = base.tables
+        same.tables = {**t, **{k: np.tile(t[k], 4) for k in ("f_val", "f_der", "phi_val", "phi_der")},
+                       **{k: np.tile(t[k], 2) for k in ("F_val", "F_der")}}
+    f1, e1, v1 = Oracle(same).compute_forces()
+    f0, e0, v0 = Oracle(base).compute_forces()
+    assert np.array_equal(f1, f0) and np.array_equal(e1, e0)
+    # (b) swapping the labels 0 <-> 1 together with the parameter blocks changes nothing
+    sw = workloads.Workload(**{**w.__dict__})
+    sw.types = (1 - w.types).astype(np.int32)
+    sw.mass = w.mass[::-1].copy()
+    if cfg == "0":
+        sw.tbsma = {k: (w.tbsma[k][[3, 2, 1, 0]] if k != "taper_on" else w.tbsma[k]) for k in w.tbsma}
+    else:
+        t, nr, nrho = w.tables, w.tables["nr"], w.tables["nrho"]
+        blk = lambda a, n, order: np.concatenate([a[i * n:(i + 1) * n] for i in order])
+        sw.tables = {**t, **{k: blk(t[k], nr, [3, 2, 1, 0]) for k in ("f_val", "f_der", "phi_val", "phi_der")},
+                     **{k: blk(t[k], nrho, [1, 0]) for k in ("F_val", "F_der")}}
+    fa, ea, va = Oracle(w).compute_forces()
+    fb, eb, vb = Oracle(sw).compute_forces()
+    assert np.array_equal(fa, fb) and np.array_equal(ea, eb)
+    assert not np.allclose(fa, f0, atol=1e-3)            # and the alloy is not the one-species system
+    # (c) alloy forces sum to zero and the run conserves momentum with two masses
+    assert np.abs(fa.sum(0)).max() < 1e-11
+    o = Oracle(w)
+    p0 = (o.velocities() * w.mass[w.types][:, None]).sum(0)
+    o.step(20, w.dt)
+    p1 = (o.velocities() * w.mass[w.types][:, None]).sum(0)
+    assert np.abs(p1 - p0).max() < 1e-12 * np.abs(o.velocities() * w.mass[w.types][:, None]).sum()

@@ -168,7 +168,7 @@ def bcc_eam(ncell: int, a: float, re: float, cutoff: float, element: str, skin: 
     sites = lattice_sites("bcc", a, (ncell,) * 3)
     rng = np.random.Generator(np.random.PCG64(seed))
     pos, vel = _jitter_and_velocities(rng, sites, sigma, MASS_AMU[element], temperature)
-    meta = dict(lattice="bcc", a=a, ncell=ncell, sigma=sigma, temperature=temperature, seed=seed)
+    meta = dict(lattice="bcc", a=a, ncell=ncell, sigma=sigma, temperature=temperature, seed=seed, re=re)
     if pka_ev > 0.0:
         u = rng.standard_normal(3)
         u /= np.sqrt((u * u).sum())
@@ -218,6 +218,37 @@ def config(k: int | str, scale: int | None = None, replica: int = 0) -> Workload
         return bcc_eam(scale or 128, 3.165, 2.741, 5.5, "W", temperature=1500.0, seed=BASE_SEED + 4, dt=0.2,
                        steps=200, pka_ev=2000.0, name="cfg4_w_bcc128_eam_pka")
     raise ValueError(f"unknown config {k!r}")
+
+
+def alloy(w: Workload, seed: int, fraction: float = 0.5) -> Workload:
+    """Binary alloy on the sites of `w` (the paper's rho^(ab), V^(ab)):
+    a seeded `fraction` of the atoms becomes type 1.  TB-SMA: type 1 gets a second, synthetic parameter set (larger
+    atom, different stiffness) and the cross pair (0,1) = (1,0) its own set, so that every entry of the 2x2 parameter
+    arrays differs; tables: the three pair tables are the analytic EAM with different (re, beta, A, B) and the two
+    embedding tables differ in F0.  Parameter arrays are indexed [ti * n_types + tj]."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    types = (rng.random(w.n_atoms) < fraction).astype(np.int32)
+    w2 = Workload(**{**w.__dict__})
+    w2.types = types
+    w2.mass = np.array([w.mass[0], 1.7 * w.mass[0]])
+    w2.name = w.name + "_alloy"
+    if w.pot_kind == 0:
+        a = {k: float(w.tbsma[k][0]) for k in ("A", "xi", "p", "q", "r0")}
+        b = dict(A=1.2 * a["A"], xi=0.96 * a["xi"], p=0.997 * a["p"], q=1.38 * a["q"], r0=1.06 * a["r0"])     # type 1
+        c = dict(A=1.09 * a["A"], xi=0.985 * a["xi"], p=1.01 * a["p"], q=1.17 * a["q"], r0=1.03 * a["r0"])    # cross
+        w2.tbsma = {k: np.array([a[k], c[k], c[k], b[k]]) for k in a}
+        w2.tbsma["taper_on"] = w.tbsma["taper_on"]
+    else:
+        t = w.tables
+        re = w.meta.get("re", 2.4725)
+        rc = t["dr"] * (t["nr"] - 1)
+        t11 = eam_tables(1.05 * re, rc, nr=t["nr"], nrho=t["nrho"], beta=5.5, A=0.45, B=0.62, F0=2.9)
+        t01 = eam_tables(1.02 * re, rc, nr=t["nr"], nrho=t["nrho"], beta=5.8, A=0.42, B=0.61)
+        pair = lambda k: np.concatenate([t[k], t01[k], t01[k], t11[k]])
+        w2.tables = dict(nr=t["nr"], dr=t["dr"], nrho=t["nrho"], drho=t["drho"],
+                         f_val=pair("f_val"), f_der=pair("f_der"), phi_val=pair("phi_val"), phi_der=pair("phi_der"),
+                         F_val=np.concatenate([t["F_val"], t11["F_val"]]), F_der=np.concatenate([t["F_der"], t11["F_der"]]))
+    return w2
 
 
 def permuted(w: Workload, seed: int) -> tuple[Workload, np.ndarray]:
