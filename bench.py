@@ -46,13 +46,23 @@ IN_CUTOFF = {"0": 42, "1": 58, "2": 42, "3a": 42, "3": 42, "3b": 86, "4": 58}
 # bounded oracle sample: unit cells per edge (boxes for config 2) of the reduced system of the same kind
 SAMPLE_SCALE = {"0": 6, "1": 24, "2": 64, "3a": 24, "3": 24, "3b": 20, "4": 24}
 
-# Algorithmic FP64-pipe instruction counts: per LISTED pair and pass the distance test;
-# per IN-CUTOFF pair the potential terms.  TB-SMA: sqrt + 1 (density) or 2 (force) exp + quintic switch;
-# tables: sqrt + 1 (density) or 2 (force) cubic-Hermite evaluations with derivative.
+# Algorithmic FP64-pipe instruction counts: the FP64 instructions that the formulas need per
+# pair in the best formulation known to this repo (FMA = 1), counted on USEFUL pairs only (lanes that idle in a
+# ragged warp, parked skin pairs and loop overhead are not work).  Per LISTED pair and pass: the distance test; per
+# IN-CUTOFF pair: the potential terms.  TB-SMA: rsqrt (5) + r (1) + one (density) or two (force) exp of 11 + quintic
+# switch (6 / 10) + combine; tables: rsqrt + r + index (2) + one or two cubic-Hermite polynomials + combine.
+# SURVEY.md section 8(d) estimated 13 / 45 / 95 before any kernel existed; round 1 replaced the estimate by these
+# counts, read off the SASS of the committed kernels, so that `frac` tracks ncu's FP64-pipe utilisation.
 SLOTS = {
-    0: dict(dist=9, dens=45, force=95),     # MD_POT_TBSMA
-    1: dict(dist=9, dens=25, force=60),     # MD_POT_EAM_TABLE
+    0: dict(dist=6, dens=25, force=48),     # MD_POT_TBSMA   (r2 with two FMAs: reading A3 only binds the list build)
+    1: dict(dist=8, dens=11, force=18),     # MD_POT_EAM_TABLE (canonical r2: the strict cut-off test decides a step)
 }
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two passes, from the committed `ncu --set full`
+# capture of this command on this workload (profiles/r01h_ncu_cfg3a.md); None for workloads without a capture.
+NCU_TRAFFIC = {"3a": {"force": 340.1e6, "density": 312.5e6, "fp64_pipe_active_pct": {"force": 50.3, "density": 41.9},
+                      "source": "profiles/r01h_ncu_cfg3a.md"}}
 
 
 def algorithmic(kind: int, n_atoms: int, list_entries: float, in_cutoff: float) -> dict:
@@ -207,6 +217,8 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
     w = workloads.config(args.workload, scale=args.scale, replica=rank)
     K, W = args.steps, args.warmup
     g = md.MDSystem(w)
+    if args.no_graph:
+        g.set_option(md.MD_OPT_GRAPH, 0)
     stream = torch.cuda.current_stream()
 
     # ---- device-resident run: W warm-up steps, then exactly K timed steps ------------------------------
@@ -250,7 +262,9 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
     roofline = {
         "kernel": "k_force (force pass + fused second half-kick)", "bound": "alu",
         "achieved": alg["force_slots"] / (f_ms * 1e-3) / 1e12, "peak": dfma_rate / 1e12, "unit": "T FP64-inst/s",
-        "frac": alg["force_slots"] / (f_ms * 1e-3) / dfma_rate, "traffic": None,
+        "frac": alg["force_slots"] / (f_ms * 1e-3) / dfma_rate,
+        "traffic": NCU_TRAFFIC.get(args.workload, {}).get("force") if args.scale is None else None,
+        "ncu": NCU_TRAFFIC.get(args.workload) if args.scale is None else None,
         "peak_source": f"md_fp64_dfma_rate measured in this run at {dfma_mhz:.0f} MHz",
         "ms_per_launch": f_ms, "algorithmic_fp64_inst_per_launch": alg["force_slots"],
         "hbm": {"achieved": alg["force_bytes"] / (f_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
@@ -326,6 +340,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="cap on the end-to-end steps (0: same as --steps)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="plain kernel launches instead of one CUDA graph per step (for ncu launch lists: ncu does not list "
+                         "kernels launched from a graph with a conditional node)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps
