@@ -191,9 +191,10 @@ __device__ __forceinline__ void hermite_nodes(const double *__restrict__ val, co
   dH = (d0 + t * (2.0 * c2 + 3.0 * t * c3)) * inv_h;
 }
 
-__device__ __forceinline__ double4 ldg4(const double4 *p) {
-  const double2 a = __ldg((const double2 *)p), b = __ldg((const double2 *)p + 1);
-  return make_double4(a.x, a.y, b.x, b.y);
+__device__ __forceinline__ double4 ldg4(const double4 *p) {       // one 256-bit load (LDG.E.256) on the read-only path
+  double4 v;
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
 }
 
 // interval index and fractional coordinate on the r grid
