@@ -130,6 +130,13 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
  * decision is taken on the device. */
 int md_step(md_system *s, int n, double dt);
 
+/* Electron-bath thermostat of eq.(4) (Finnis et al.):  m dv/dt = f - (m/tau)((T_i - T_e)/T_i) v  with the
+ * per-atom instantaneous temperature T_i = m |v|^2 / (3 k_B).  T_e in K, tau in fs (a time: the printed 1/tau_T stands
+ * for m_i/tau_T); tau <= 0 switches it off (default).  Inside md_step each half-kick becomes
+ * v += (dt/2)(f/m - (1/tau)(1 - 3 k_B T_e/(m |v|^2)) v), the damping taken from the velocity the half-kick starts from,
+ * and 0 for an atom at rest.  Returns MD_EINVAL for T_e < 0 or non-finite arguments. */
+int md_set_thermostat(md_system *s, double T_e, double tau);
+
 int md_get_positions(md_system *s, double *x);        /* [n_atoms][3]; as wrapped at the last build plus drift since */
 int md_get_velocities(md_system *s, double *v);       /* [n_atoms][3] */
 int md_set_positions(md_system *s, const double *x);  /* keeps the list if no atom is farther than skin/2 from x_ref */
@@ -149,7 +156,8 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                              (the paper's full-MD runs).  md_compute_forces always computes them.
  *  MD_OPT_PROFILE           1: bracket every kernel launch with CUDA events on the system's stream so that
  *                              md_profile_read can report per-kernel device time.
- *  MD_OPT_FORCE_VARIANT     0: choose by neighbour count; 1: thread-per-atom; 2: warp-per-atom.
+ *  MD_OPT_FORCE_VARIANT     0: choose by system size (8 lanes per atom up to 24,576 atoms); 1: one thread per atom;
+ *                           2: 8 lanes per atom.
  *  MD_OPT_GRAPH             1 (default): md_step replays one CUDA graph per time step whose neighbour rebuild is
  *                           the body of a conditional node (4 kernel launches per step when no rebuild is due);
  *                           0: plain launches (every kernel of the rebuild chain is launched and returns at once

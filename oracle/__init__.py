@@ -48,6 +48,7 @@ def lib():
         _lib.oracle_tbsma_eval.argtypes = [C.c_double] * 8 + [_D]
         _lib.oracle_min_image.argtypes = [_D, _D, _D, _D, _D]
         _lib.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        _lib.oracle_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
     return _lib
 
 
@@ -143,6 +144,10 @@ class Oracle:
 
     def step(self, n: int, dt: float):
         self._check(lib().oracle_step(self._h, int(n), float(dt)))
+
+    def set_thermostat(self, T_e: float, tau: float):
+        """eq.(4): electron-bath thermostat (K, fs); tau <= 0 switches it off."""
+        self._check(lib().oracle_set_thermostat(self._h, float(T_e), float(tau)))
 
     def positions(self):
         x = np.zeros((self.n_atoms, 3))

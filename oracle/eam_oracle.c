@@ -26,6 +26,7 @@
 struct oracle_system {
   int N, nb, npb, nt;
   double L[3], rc, skin, rl, rc2, rl2;
+  double thermo_Te, thermo_tau;          /* electron-bath thermostat, eq.(4); tau <= 0: off */
   double *x, *v, *f, *xref, *m;          /* m: per type, eV fs^2/A^2 */
   int *type;
   int kind;
@@ -355,9 +356,32 @@ int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, doub
   return ORACLE_OK;
 }
 
+/* Electron-bath thermostat, eq.(4):  m dv/dt = f - (m/tau_T) ((T_i - T_e)/T_i) v,  with the per-atom
+ * instantaneous temperature T_i = m |v|^2 / (3 k_B).  Reading (T1): tau_T is a time, so the printed 1/tau_T
+ * stands for m_i/tau_T; the damping acceleration is -(1/tau_T)(1 - c2/|v|^2) v with c2 = 3 k_B T_e / m_i, and 0 for an
+ * atom at rest.  Each half-kick of the velocity-Verlet step uses the damping of the velocity it starts from. */
+#define KB_EV 8.617333262e-5
+int oracle_set_thermostat(oracle_system *s, double T_e, double tau) {
+  if (!s || !(T_e >= 0.0)) return ORACLE_EINVAL;
+  s->thermo_Te = T_e; s->thermo_tau = tau;
+  return ORACLE_OK;
+}
+
+static void half_kick(oracle_system *s, int i, double dt) {
+  const double m = s->m[s->type[i]], h = 0.5 * dt / m;
+  double *v = s->v + 3 * i;
+  const double *f = s->f + 3 * i;
+  double g = 0.0;
+  if (s->thermo_tau > 0.0) {
+    const double v2 = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
+    if (v2 > 0.0) g = (1.0 / s->thermo_tau) * (1.0 - (3.0 * KB_EV * s->thermo_Te / m) / v2);
+  }
+  for (int a = 0; a < 3; ++a) v[a] = v[a] + h * f[a] - (0.5 * dt * g) * v[a];
+}
+
 /* Velocity-Verlet (BASELINE.json north_star) with the skin/2 rule (readings A10, A11):
- *   v += (dt/2m) f; x += dt v; if max_i |x_i - x_ref,i|^2 > (skin/2)^2: rebuild;
- *   f <- force(x); v += (dt/2m) f. */
+ *   v += (dt/2)(f/m + a_fric(v)); x += dt v; if max_i |x_i - x_ref,i|^2 > (skin/2)^2: rebuild;
+ *   f <- force(x); v += (dt/2)(f/m + a_fric(v)). */
 int oracle_step(oracle_system *s, int n, double dt) {
   int rc;
   if (!s || n < 0) return ORACLE_EINVAL;
@@ -368,9 +392,9 @@ int oracle_step(oracle_system *s, int n, double dt) {
   for (int step = 0; step < n; ++step) {
     double maxd2 = 0.0;
     for (int i = 0; i < N; ++i) {
-      double h = 0.5 * dt / s->m[s->type[i]], d2 = 0.0;
+      double d2 = 0.0;
+      half_kick(s, i, dt);
       for (int a = 0; a < 3; ++a) {
-        s->v[3 * i + a] += h * s->f[3 * i + a];
         s->x[3 * i + a] += dt * s->v[3 * i + a];
         double u = s->x[3 * i + a] - s->xref[3 * i + a];
         d2 += u * u;
@@ -381,10 +405,7 @@ int oracle_step(oracle_system *s, int n, double dt) {
     s->st.last_max_disp2 = maxd2;
     if (maxd2 > thr && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
     if ((rc = forces_internal(s)) != ORACLE_OK) return rc;
-    for (int i = 0; i < N; ++i) {
-      double h = 0.5 * dt / s->m[s->type[i]];
-      for (int a = 0; a < 3; ++a) s->v[3 * i + a] += h * s->f[3 * i + a];
-    }
+    for (int i = 0; i < N; ++i) half_kick(s, i, dt);
     s->st.steps += 1;
   }
   return ORACLE_OK;

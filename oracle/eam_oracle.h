@@ -59,6 +59,8 @@ int oracle_set_threads(int n);                           /* OpenMP threads; retu
 int oracle_build_neighbors(oracle_system *s, int mode);
 int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, double *virial /*[n_boxes][6]*/);
 int oracle_step(oracle_system *s, int n, double dt);
+/* eq.(4): electron-bath thermostat at temperature T_e (K) with time constant tau (fs); tau <= 0: off */
+int oracle_set_thermostat(oracle_system *s, double T_e, double tau);
 int oracle_get_positions(oracle_system *s, double *x);
 int oracle_get_velocities(oracle_system *s, double *v);
 int oracle_set_positions(oracle_system *s, const double *x);

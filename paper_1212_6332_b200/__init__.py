@@ -75,6 +75,7 @@ def lib() -> C.CDLL:
         L.md_get_energies.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_get_stats.argtypes = [C.c_void_p, C.POINTER(MdStats)]
         L.md_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.md_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.md_profile_read.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_long), C.POINTER(C.c_double)]
         L.md_fp64_dfma_rate.argtypes = [C.c_void_p, _D, _D]
         _lib = L
@@ -235,6 +236,10 @@ class MDSystem:
         st = MdStats()
         check(lib().md_get_stats(self._h, C.byref(st)))
         return {k: getattr(st, k) for k, _ in MdStats._fields_}
+
+    def set_thermostat(self, T_e: float, tau: float):
+        """eq.(4) electron-bath thermostat (K, fs); tau <= 0 switches it off."""
+        check(lib().md_set_thermostat(self._h, float(T_e), float(tau)))
 
     def set_option(self, option: int, value: int):
         check(lib().md_set_option(self._h, int(option), int(value)))

@@ -411,6 +411,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
   s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
+  s->thermo_Te = 0.0; s->thermo_tau = 0.0;
   s->step_graph = nullptr; s->step_exec = nullptr; s->step_dt = 0.0; s->step_obs = false; s->step_kernels = s->body_kernels = 0;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
@@ -516,6 +517,13 @@ int md_set_option(md_system *s, int option, int value) {
     case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
   }
   return MD_EINVAL;
+}
+
+int md_set_thermostat(md_system *s, double T_e, double tau) {
+  if (!s || !(T_e >= 0.0) || !isfinite(T_e) || !isfinite(tau)) return MD_EINVAL;
+  s->thermo_Te = T_e; s->thermo_tau = tau;
+  drop_step_graph(s);                                // the half-kick parameters are baked into the graph's nodes
+  return MD_OK;
 }
 
 int md_build_neighbors(md_system *s) {

@@ -444,7 +444,6 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
 // OBS: also E_i = F(rho_i) + 1/2 sum_j V(r) [eq.(1)] and W^{ab} = -1/2 sum_j s_ij d^a d^b / r.
 // kick.h[type] != 0: second half-kick v += (dt/2m) f fused into the epilogue.
 // ------------------------------------------------------------------------------------------------
-struct KickParams { double h[MD_MAX_TYPES]; };
 
 template <bool OBS> struct ForceAcc;
 template <> struct ForceAcc<false> { double fx = 0.0, fy = 0.0, fz = 0.0; };
@@ -529,8 +528,11 @@ __device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &
   if (valid) {
     const size_t N = (size_t)s.N;
     s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
-    const double h = kick.h[ti];
-    if (h != 0.0) { s.vel[i] += h * acc.fx; s.vel[N + i] += h * acc.fy; s.vel[2 * N + i] += h * acc.fz; }
+    if (kick.h[ti] != 0.0) {
+      double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
+      half_kick(kick, ti, acc.fx, acc.fy, acc.fz, vx, vy, vz);
+      s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
+    }
     if (!(fabs(acc.fx) + fabs(acc.fy) + fabs(acc.fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
   }
   if constexpr (OBS) {
@@ -842,8 +844,7 @@ static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams 
 }
 
 int launch_force(md_system *sys, bool observables, double half_dt) {
-  KickParams kp;
-  for (int t = 0; t < MD_MAX_TYPES; ++t) kp.h[t] = (t < sys->d.nt) ? half_dt / sys->mass_ev[t] : 0.0;
+  const KickParams kp = make_kick(sys, half_dt);
   const int grid = force_blocks(sys);
   {
     ProfScope p(sys, MD_K_FORCE);

@@ -8,19 +8,17 @@
 
 namespace md {
 
-struct DtParams { double dt; double h[MD_MAX_TYPES]; };   // h = dt/(2m) per type
 
 // v += (dt/2m) f;  x += dt v;  d2 = |x - x_ref|^2  -> block max -> atomicMax on the bit pattern.
-__global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ DevSys s, const DtParams p) {
+__global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ DevSys s, const KickParams p, double dt) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const size_t N = (size_t)s.N;
   double d2 = 0.0;
   if (i < s.N) {
     double4 x = s.pos[i];
-    const double h = p.h[s.nt > 1 ? (int)x.w : 0];
     double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
-    vx += h * s.frc[i]; vy += h * s.frc[N + i]; vz += h * s.frc[2 * N + i];
-    x.x += p.dt * vx; x.y += p.dt * vy; x.z += p.dt * vz;
+    half_kick(p, s.nt > 1 ? (int)x.w : 0, s.frc[i], s.frc[N + i], s.frc[2 * N + i], vx, vy, vz);
+    x.x += dt * vx; x.y += dt * vy; x.z += dt * vz;
     s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
     s.pos[i] = x;
     const double ux = x.x - s.xref[i], uy = x.y - s.xref[N + i], uz = x.z - s.xref[2 * N + i];
@@ -41,12 +39,22 @@ __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ DevS
   }
 }
 
+KickParams make_kick(const md_system *sys, double half_dt) {
+  KickParams k;
+  const bool on = sys->thermo_tau > 0.0 && half_dt != 0.0;
+  k.gdt = on ? half_dt / sys->thermo_tau : 0.0;
+  for (int t = 0; t < MD_MAX_TYPES; ++t) {
+    const bool used = t < sys->d.nt;
+    k.h[t] = used ? half_dt / sys->mass_ev[t] : 0.0;
+    k.c2[t] = used ? 3.0 * kBoltzmannEv * sys->thermo_Te / sys->mass_ev[t] : 0.0;
+  }
+  return k;
+}
+
 int launch_kick_drift(md_system *sys, double dt) {
   ProfScope p(sys, MD_K_INTEGRATE);
-  DtParams dp;
-  dp.dt = dt;
-  for (int t = 0; t < MD_MAX_TYPES; ++t) dp.h[t] = (t < sys->d.nt) ? 0.5 * dt / sys->mass_ev[t] : 0.0;
-  ++sys->launches, k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, dp);
+  const KickParams kp = make_kick(sys, 0.5 * dt);
+  ++sys->launches, k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, kp, dt);
   return (int)cudaGetLastError();
 }
 

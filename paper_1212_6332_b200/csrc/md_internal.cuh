@@ -100,6 +100,7 @@ struct md_system {
   cudaStream_t stream;
   double mass_ev[MD_MAX_TYPES];    // eV fs^2 / A^2
   double cutoff, skin;
+  double thermo_Te, thermo_tau;    // eq.(4) thermostat; tau <= 0: off
   bool have_list, forces_valid, observables_valid;
   bool opt_step_obs, opt_profile, opt_graph;
   // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
@@ -113,6 +114,20 @@ struct md_system {
 };
 
 namespace md {
+constexpr double kBoltzmannEv = 8.617333262e-5;     // eV/K
+// half-kick parameters: h[t] = dt/(2 m_t); thermostat (eq.4): gdt = dt/(2 tau) (0: off), c2[t] = 3 k_B T_e / m_t
+struct KickParams { double h[MD_MAX_TYPES]; double c2[MD_MAX_TYPES]; double gdt; };
+KickParams make_kick(const md_system *s, double half_dt);
+// v <- v + h f - gdt (1 - c2/|v|^2) v   (the second term only with the thermostat on; 0 for an atom at rest)
+__device__ __forceinline__ void half_kick(const KickParams &k, int t, double fx, double fy, double fz, double &vx, double &vy, double &vz) {
+  double g = 0.0;
+  if (k.gdt != 0.0) {
+    const double v2 = (vx * vx + vy * vy) + vz * vz;
+    if (v2 > 0.0) g = k.gdt * (1.0 - k.c2[t] / v2);
+  }
+  const double h = k.h[t];
+  vx = vx + h * fx - g * vx; vy = vy + h * fy - g * vy; vz = vz + h * fz - g * vz;
+}
 // launch geometry of the per-atom kernels that use the tile mapping
 constexpr int kForceBlock = 128;
 constexpr int kSubMaxAtoms = 24576;                // at or below this many atoms the passes use 8 lanes per atom (md_force.cu)

@@ -176,6 +176,39 @@ def test_graph_step_equals_plain_launches(md, case):
     assert np.array_equal(a.positions(), b.positions())
 
 
+@pytest.mark.parametrize("case,variant", [("cfg0", 0), ("alloy_tbsma", 1), ("alloy_tables", 2), ("cfg2_small", 0)])
+def test_thermostat_trajectory(md, case, variant):
+    """eq.(4) electron-bath thermostat (row f1): same half-kicks as the oracle, through the graph and the plain path."""
+    w = CASES[case]()
+    o = oracle_of(w)
+    g = md.MDSystem(w)
+    g.set_option(md.MD_OPT_FORCE_VARIANT, variant)
+    g.step(10, w.dt)                                   # first without: setting the thermostat must re-build the step graph
+    o.step(10, w.dt)
+    for x in (o, g):
+        x.set_thermostat(900.0, 60.0)
+    o.step(90, w.dt)
+    g.step(90, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL
+    assert np.abs(g.velocities() - o.velocities()).max() <= 1e-9
+    ek_o, ek_g = o.energies()[1].sum(), g.energies()[1].sum()
+    assert abs(ek_g - ek_o) <= 1e-10 * ek_o
+    # the bath is hotter than the crystal: it has heated up, and switching the thermostat off restores plain NVE steps
+    w0 = CASES[case]()
+    ref = oracle_of(w0); ref.step(100, w.dt)
+    assert ek_o > 1.05 * ref.energies()[1].sum()
+    for x in (o, g):
+        x.set_thermostat(0.0, 0.0)
+    o.step(10, w.dt); g.step(10, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+    with pytest.raises(md.MDError):
+        g.set_thermostat(-1.0, 10.0)
+
+
 def test_run_to_run_determinism(md):
     w = CASES["cfg2_small"]()
     res = []

@@ -517,3 +517,66 @@ def test_alloy_reduces_to_one_species_and_label_swap(cfg):
     o.step(20, w.dt)
     p1 = (o.velocities() * w.mass[w.types][:, None]).sum(0)
     assert np.abs(p1 - p0).max() < 1e-12 * np.abs(o.velocities() * w.mass[w.types][:, None]).sum()
+
+
+# ---------------------------------------------------------------- electron-bath thermostat, eq.(4)
+KB = 8.617333262e-5
+AMU = 103.642696526805
+
+
+def _free_atoms(speeds, masses=(63.546, 107.8682)):
+    """atoms further apart than the cut-off (no forces), two species, prescribed speeds along random directions"""
+    n = len(speeds)
+    rng = np.random.default_rng(8)
+    grid = np.array([[i, j, k] for i in range(3) for j in range(3) for k in range(3)], float)[:n] * 13.0 + 3.0
+    u = rng.standard_normal((n, 3)); u /= np.linalg.norm(u, axis=1)[:, None]
+    types = (np.arange(n) % 2).astype(np.int32)
+    tb = workloads.alloy(workloads.config(0, scale=5), 1).tbsma
+    return dict(pot_kind=0, mass=np.array(masses), tbsma=tb, box=np.full(3, 39.0), positions=grid, cutoff=4.9, skin=0.3,
+                velocities=u * np.asarray(speeds)[:, None], types=types, n_boxes=1), types
+
+
+def test_thermostat_free_atoms_closed_form():
+    """no forces: |v|^2(t) = c2 + (|v0|^2 - c2) exp(-2t/tau), c2 = 3 k_B T_e/m, direction unchanged; first order in dt"""
+    Te, tau, T = 450.0, 80.0, 120.0
+    speeds = np.array([0.001, 0.004, 0.008, 0.002, 0.012, 0.0005, 0.006, 0.003])
+    kw, types = _free_atoms(speeds)
+    m = np.array(kw["mass"])[types] * AMU
+    c2 = 3 * KB * Te / m
+    exact = np.sqrt(c2 + (speeds ** 2 - c2) * np.exp(-2 * T / tau))
+    err = []
+    for dt in (0.5, 0.25):
+        o = Oracle(**kw)
+        o.set_thermostat(Te, tau)
+        o.step(int(round(T / dt)), dt)
+        v = o.velocities()
+        s = np.linalg.norm(v, axis=1)
+        assert np.abs(np.cross(v / s[:, None], kw["velocities"] / speeds[:, None])).max() < 1e-12     # same direction
+        err.append(np.abs(s - exact).max())
+        assert err[-1] < 2e-2 * exact.max() * dt
+    assert 1.7 < err[0] / err[1] < 2.3
+    # atoms hotter than the bath slow down, colder ones speed up
+    assert np.all((s < speeds) == (speeds ** 2 > c2))
+
+
+def test_thermostat_off_limits_and_crystal_temperature():
+    w = workloads.config(0, scale=5)
+    a, b, c = Oracle(w), Oracle(w), Oracle(w)
+    b.set_thermostat(300.0, 1e30)                       # infinitely slow exchange == no thermostat
+    c.set_thermostat(300.0, 0.0)                        # tau <= 0: off
+    for o in (a, b, c):
+        o.step(30, 1.0)
+    assert np.abs(a.positions() - b.positions()).max() < 1e-13 and np.array_equal(a.positions(), c.positions())
+    # a 300 K crystal coupled to a 900 K bath heats up towards it (equipartition halves the initial kinetic T first)
+    o = Oracle(w)
+    o.set_thermostat(900.0, 40.0)
+    o.step(600, 1.0)
+    temps = []
+    for _ in range(10):
+        o.step(20, 1.0)
+        temps.append(2 * o.energies()[1].sum() / (3 * w.n_atoms * KB))
+    assert 750.0 < np.mean(temps) < 1050.0
+    # an atom at rest feels no damping (no division by zero)
+    kw, _ = _free_atoms(np.array([0.0, 0.002]))
+    o = Oracle(**kw); o.set_thermostat(300.0, 50.0); o.step(5, 1.0)
+    assert np.all(o.velocities()[0] == 0.0) and np.all(np.isfinite(o.velocities()))
