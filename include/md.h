@@ -56,7 +56,7 @@ enum {
 };
 
 /* bits of md_stats.error_flags */
-enum { MD_FLAG_OVERFLOW = 1, MD_FLAG_NONFINITE = 2 };
+enum { MD_FLAG_OVERFLOW = 1, MD_FLAG_NONFINITE = 2, MD_FLAG_BOX = 4 /* barostat shrank a cell below cutoff + skin */ };
 
 enum { MD_POT_TBSMA = 0, MD_POT_EAM_TABLE = 1 };
 enum { MD_MAX_TYPES = 4 };
@@ -136,6 +136,17 @@ int md_step(md_system *s, int n, double dt);
  * v += (dt/2)(f/m - (1/tau)(1 - 3 k_B T_e/(m |v|^2)) v), the damping taken from the velocity the half-kick starts from,
  * and 0 for an atom at rest.  Returns MD_EINVAL for T_e < 0 or non-finite arguments. */
 int md_set_thermostat(md_system *s, double T_e, double tau);
+
+/* Berendsen barostat of eq.(5)-(6): at the end of every step of md_step the coordinates and the box
+ * edges are scaled by mu = [1 - (dt/tau_p)(P0 - P)]^(1/3), P = (2/3 E_kin + 1/3 (W_xx + W_yy + W_zz)) / V from the force
+ * evaluation of that step (which then always computes the observables).  P0 in eV/A^3, tau_p in fs eV/A^3 (it absorbs
+ * the compressibility); tau_p <= 0 switches it off (default).  One box only (MD_EINVAL for n_boxes > 1).  The cell grid
+ * keeps the number of cells chosen at md_create: if the box shrinks until a cell is thinner than cutoff + skin the
+ * sticky flag MD_FLAG_BOX is raised and the next synchronising call returns MD_EBOX.  x_ref is not scaled, so the
+ * skin/2 rebuild rule also sees the displacement caused by the scaling. */
+int md_set_barostat(md_system *s, double P0, double tau_p);
+int md_get_box(md_system *s, double *box /* [3] host */);                /* current box edges; synchronises */
+int md_get_pressure(md_system *s, double *P /* host, eV/A^3 */);         /* eq.(6) for the current state; synchronises */
 
 int md_get_positions(md_system *s, double *x);        /* [n_atoms][3]; as wrapped at the last build plus drift since */
 int md_get_velocities(md_system *s, double *v);       /* [n_atoms][3] */

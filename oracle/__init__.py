@@ -49,6 +49,9 @@ def lib():
         _lib.oracle_min_image.argtypes = [_D, _D, _D, _D, _D]
         _lib.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _lib.oracle_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        _lib.oracle_set_barostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        _lib.oracle_get_box.argtypes = [C.c_void_p, _D]
+        _lib.oracle_get_pressure.argtypes = [C.c_void_p, _D]
     return _lib
 
 
@@ -148,6 +151,20 @@ class Oracle:
     def set_thermostat(self, T_e: float, tau: float):
         """eq.(4): electron-bath thermostat (K, fs); tau <= 0 switches it off."""
         self._check(lib().oracle_set_thermostat(self._h, float(T_e), float(tau)))
+
+    def set_barostat(self, P0: float, tau_p: float):
+        """eq.(5)-(6): Berendsen barostat (eV/A^3, fs eV/A^3); tau_p <= 0 switches it off."""
+        self._check(lib().oracle_set_barostat(self._h, float(P0), float(tau_p)))
+
+    def box(self):
+        b = np.zeros(3)
+        self._check(lib().oracle_get_box(self._h, _dp(b)))
+        return b
+
+    def pressure(self) -> float:
+        p = C.c_double()
+        self._check(lib().oracle_get_pressure(self._h, C.byref(p)))
+        return p.value
 
     def positions(self):
         x = np.zeros((self.n_atoms, 3))

@@ -27,6 +27,8 @@ struct oracle_system {
   int N, nb, npb, nt;
   double L[3], rc, skin, rl, rc2, rl2;
   double thermo_Te, thermo_tau;          /* electron-bath thermostat, eq.(4); tau <= 0: off */
+  double baro_P0, baro_tau;              /* Berendsen barostat, eq.(5); tau <= 0: off */
+  int obs_stale;                         /* the barostat scaled x after the last force evaluation */
   double *x, *v, *f, *xref, *m;          /* m: per type, eV fs^2/A^2 */
   int *type;
   int kind;
@@ -288,6 +290,7 @@ int oracle_build_neighbors(oracle_system *s, int mode) {
 
 /* Density pass (Fig.5 G18) then force pass (Fig.6 G22). */
 static int forces_internal(oracle_system *s) {
+  s->obs_stale = 0;
   const int N = s->N;
   int bad = 0;
   /* G18: rho_i = sum_{j in list, r < r_c} f(r_ij); then F(rho_i), F'(rho_i) */
@@ -367,6 +370,35 @@ int oracle_set_thermostat(oracle_system *s, double T_e, double tau) {
   return ORACLE_OK;
 }
 
+/* Berendsen barostat, eq.(5)-(6): at the end of every step the coordinates and the box edges are
+ * scaled by mu = [1 - (dt/tau_p)(P_0 - P)]^(1/3), with P = (N k_B T + 1/3 sum_i f_i.r_i)/V.  Readings (B1):
+ * N k_B T = 2/3 E_kin (velocities after the second half-kick), the virial sum is the pairwise trace W_xx+W_yy+W_zz of
+ * the force evaluation of this step, V = Lx Ly Lz; pressures in eV/A^3, tau_p in fs eV/A^3 (it absorbs the
+ * compressibility); x_ref is NOT scaled, so the skin/2 rule also sees the displacement that the scaling causes. */
+int oracle_set_barostat(oracle_system *s, double P0, double tau_p) {
+  if (!s || (tau_p > 0.0 && s->nb != 1)) return ORACLE_EINVAL;
+  s->baro_P0 = P0; s->baro_tau = tau_p;
+  return ORACLE_OK;
+}
+int oracle_get_box(oracle_system *s, double *box) { for (int a = 0; a < 3; ++a) box[a] = s->L[a]; return ORACLE_OK; }
+
+static double pressure_now(const oracle_system *s) {
+  long double ek = 0;
+  for (int i = 0; i < s->N; ++i) {
+    const double *v = s->v + 3 * i;
+    ek += 0.5 * s->m[s->type[i]] * ((v[0] * v[0] + v[1] * v[1]) + v[2] * v[2]);
+  }
+  const double trw = (s->virial[0] + s->virial[1]) + s->virial[2];
+  return ((2.0 / 3.0) * (double)ek + trw / 3.0) / (s->L[0] * s->L[1] * s->L[2]);
+}
+int oracle_get_pressure(oracle_system *s, double *P) {
+  int rc;
+  if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
+  if ((!s->forces_valid || s->obs_stale) && (rc = forces_internal(s)) != ORACLE_OK) return rc;
+  *P = pressure_now(s);
+  return ORACLE_OK;
+}
+
 static void half_kick(oracle_system *s, int i, double dt) {
   const double m = s->m[s->type[i]], h = 0.5 * dt / m;
   double *v = s->v + 3 * i;
@@ -406,6 +438,12 @@ int oracle_step(oracle_system *s, int n, double dt) {
     if (maxd2 > thr && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
     if ((rc = forces_internal(s)) != ORACLE_OK) return rc;
     for (int i = 0; i < N; ++i) half_kick(s, i, dt);
+    if (s->baro_tau > 0.0) {
+      const double mu = cbrt(1.0 - (dt / s->baro_tau) * (s->baro_P0 - pressure_now(s)));
+      for (int i = 0; i < 3 * N; ++i) s->x[i] *= mu;
+      for (int a = 0; a < 3; ++a) s->L[a] *= mu;
+      s->obs_stale = 1;     /* energies / pressure on request are re-evaluated; the next half-kick keeps these forces */
+    }
     s->st.steps += 1;
   }
   return ORACLE_OK;
@@ -438,7 +476,7 @@ int oracle_get_densities(oracle_system *s, double *rho, double *fp) {
 int oracle_get_energies(oracle_system *s, double *epot, double *ekin) {
   int rc;
   if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
-  if (!s->forces_valid && (rc = forces_internal(s)) != ORACLE_OK) return rc;
+  if ((!s->forces_valid || s->obs_stale) && (rc = forces_internal(s)) != ORACLE_OK) return rc;
   for (int b = 0; b < s->nb; ++b) {
     long double ep = 0, ek = 0;
     for (int i = b * s->npb; i < (b + 1) * s->npb; ++i) {

@@ -61,6 +61,10 @@ int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, doub
 int oracle_step(oracle_system *s, int n, double dt);
 /* eq.(4): electron-bath thermostat at temperature T_e (K) with time constant tau (fs); tau <= 0: off */
 int oracle_set_thermostat(oracle_system *s, double T_e, double tau);
+/* eq.(5)-(6): Berendsen barostat, P0 in eV/A^3, tau_p in fs eV/A^3; tau_p <= 0: off; one box only */
+int oracle_set_barostat(oracle_system *s, double P0, double tau_p);
+int oracle_get_box(oracle_system *s, double *box);
+int oracle_get_pressure(oracle_system *s, double *P);   /* eq.(6) for the current state, eV/A^3 */
 int oracle_get_positions(oracle_system *s, double *x);
 int oracle_get_velocities(oracle_system *s, double *v);
 int oracle_set_positions(oracle_system *s, const double *x);

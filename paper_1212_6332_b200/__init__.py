@@ -76,6 +76,9 @@ def lib() -> C.CDLL:
         L.md_get_stats.argtypes = [C.c_void_p, C.POINTER(MdStats)]
         L.md_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.md_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.md_set_barostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.md_get_box.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.md_get_pressure.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.md_profile_read.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_long), C.POINTER(C.c_double)]
         L.md_fp64_dfma_rate.argtypes = [C.c_void_p, _D, _D]
         _lib = L
@@ -240,6 +243,20 @@ class MDSystem:
     def set_thermostat(self, T_e: float, tau: float):
         """eq.(4) electron-bath thermostat (K, fs); tau <= 0 switches it off."""
         check(lib().md_set_thermostat(self._h, float(T_e), float(tau)))
+
+    def set_barostat(self, P0: float, tau_p: float):
+        """eq.(5)-(6) Berendsen barostat (eV/A^3, fs eV/A^3); tau_p <= 0 switches it off."""
+        check(lib().md_set_barostat(self._h, float(P0), float(tau_p)))
+
+    def box(self):
+        b = (C.c_double * 3)()
+        check(lib().md_get_box(self._h, b))
+        return np.array(list(b))
+
+    def pressure(self) -> float:
+        p = C.c_double()
+        check(lib().md_get_pressure(self._h, C.byref(p)))
+        return p.value
 
     def set_option(self, option: int, value: int):
         check(lib().md_set_option(self._h, int(option), int(value)))

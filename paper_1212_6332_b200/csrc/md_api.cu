@@ -198,7 +198,8 @@ __global__ void k_set_pos(const __grid_constant__ DevSys s, const double *__rest
     for (int c = 0; c < 3; ++c) {
       const double ref = s.xref[c * N + i];
       double u = x[c] - ref;
-      u -= s.L[c] * rint(u / s.L[c]);
+      const double Lc = box_edge(s, c);
+      u -= Lc * rint(u / Lc);
       x[c] = ref + u;
       d2 += u * u;
     }
@@ -248,6 +249,7 @@ static int sync_and_flags(md_system *s, int *flags_out = nullptr) {
   if (cudaMemcpyAsync(&st, s->d.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
   if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   if (flags_out) *flags_out = st.error_flags;
+  if (st.error_flags & MD_FLAG_BOX) return MD_EBOX;                 // first: an over-compressed box also overflows the lists
   if (st.error_flags & MD_FLAG_NONFINITE) return MD_ENONFINITE;
   if (st.error_flags & MD_FLAG_OVERFLOW) return MD_EOVERFLOW;
   return MD_OK;
@@ -331,6 +333,7 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
   if (ok) {
     long l0 = s->launches;
     ok = launch_density(s) == 0 && launch_force(s, obs, 0.5 * dt) == 0;
+    if (ok && s->baro_tau > 0.0) ok = launch_barostat(s, dt) == 0;
     tail = s->launches - l0;
     ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
   }
@@ -411,15 +414,16 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
   s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
-  s->thermo_Te = 0.0; s->thermo_tau = 0.0;
+  s->thermo_Te = 0.0; s->thermo_tau = 0.0; s->baro_P0 = 0.0; s->baro_tau = 0.0;
   s->step_graph = nullptr; s->step_exec = nullptr; s->step_dt = 0.0; s->step_obs = false; s->step_kernels = s->body_kernels = 0;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
   o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
   const double rl = d->cutoff + d->skin;
   for (int a = 0; a < 3; ++a) {
-    o.L[a] = d->box[a]; o.hL[a] = 0.5 * d->box[a]; o.nc[a] = g.nc[a]; o.cell_scale[a] = (double)g.nc[a] / d->box[a];
+    o.nc[a] = g.nc[a]; o.L0[a] = d->box[a];
   }
+  o.rl = rl; o.dyn_box = 0;
   o.rc2 = d->cutoff * d->cutoff; o.rin2 = o.rc2; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
   o.tnc = g.tnc; o.ncell = g.ncell; o.cap = g.cap; o.tiles_per_box = g.tiles_per_box;
   s->n_force_blocks = g.n_blocks;
@@ -427,6 +431,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   const size_t N = (size_t)o.N, nt2 = (size_t)o.nt * o.nt;
   cudaStream_t st = s->stream;
   cudaError_t e = cudaMemsetAsync(o.st, 0, sizeof(DevState), st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(o.st->box, d->box, 3 * sizeof(double), cudaMemcpyHostToDevice, st);
   {
     // 2^(j/64), j = 0..63, rounded from long double (64-bit mantissa): the table of exp_scaled() in md_force.cu
     for (int j = 0; j < 64; ++j) s->exp_tab_host[j] = (double)exp2l((long double)j / 64.0L);
@@ -526,6 +531,35 @@ int md_set_thermostat(md_system *s, double T_e, double tau) {
   return MD_OK;
 }
 
+int md_set_barostat(md_system *s, double P0, double tau_p) {
+  if (!s || !isfinite(P0) || !isfinite(tau_p) || (tau_p > 0.0 && s->d.nb != 1)) return MD_EINVAL;
+  s->baro_P0 = P0; s->baro_tau = tau_p;
+  drop_step_graph(s);                                // parameters are baked into the graph's nodes
+  if (tau_p > 0.0) s->d.dyn_box = 1;                 // kernels read the box edges from device state from now on
+  else if (s->d.dyn_box) {                           // switched off: the current edges become kernel parameters again
+    if (cudaMemcpyAsync(s->d.L0, s->d.st->box, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+        cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+    s->d.dyn_box = 0;
+  }
+  return MD_OK;
+}
+
+int md_get_box(md_system *s, double *box) {
+  if (!s || !box) return MD_EINVAL;
+  if (cudaMemcpyAsync(box, s->d.st->box, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  return sync_and_flags(s);
+}
+
+int md_get_pressure(md_system *s, double *P) {
+  if (!s || !P) return MD_EINVAL;
+  int rc;
+  if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+  if (!(s->forces_valid && s->observables_valid) && (rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+  if (launch_pressure(s) != 0) return MD_ECUDA;
+  if (cudaMemcpyAsync(P, &s->d.st->pressure, sizeof(double), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  return sync_and_flags(s);
+}
+
 int md_build_neighbors(md_system *s) {
   if (!s) return MD_EINVAL;
   int rc = request_rebuild(s);
@@ -573,17 +607,21 @@ int md_step(md_system *s, int n, double dt) {
   if (n == 0) return MD_OK;
   if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
   if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
-  if (s->opt_graph && !s->opt_profile && build_step_graph(s, dt, s->opt_step_obs) == MD_OK) {
+  const bool baro = s->baro_tau > 0.0;
+  const bool obs = s->opt_step_obs || baro;          // the barostat needs the virial of every step
+  if (s->opt_graph && !s->opt_profile && build_step_graph(s, dt, obs) == MD_OK) {
     // one graph launch per step: 4 kernels when no rebuild is due, no launch of the chain's kernels at all
     for (int k = 0; k < n; ++k)
       if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) return MD_ECUDA;
     s->launches += (long)n * s->step_kernels;
-    s->have_list = true; s->forces_valid = true; s->observables_valid = s->opt_step_obs;
+    s->have_list = true; s->forces_valid = true; s->observables_valid = obs && !baro;
   } else {
     for (int k = 0; k < n; ++k) {
       if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
-      if ((rc = forces_sequence(s, s->opt_step_obs, 0.5 * dt)) != MD_OK) return rc;
+      if ((rc = forces_sequence(s, obs, 0.5 * dt)) != MD_OK) return rc;
+      if (baro && launch_barostat(s, dt) != 0) return MD_ECUDA;
     }
+    if (baro) s->observables_valid = false;          // energies and virial on request belong to the scaled positions
   }
   s->steps += n;
   return MD_OK;

@@ -42,16 +42,17 @@ __device__ __forceinline__ double image_delta(double xj, double xi, unsigned cod
 // CANON: r2 = (dx*dx + dy*dy) + dz*dz with every operation rounded once (reading A3), needed where r2 < rc2 decides a
 // discontinuous term (tables, reading A9).  Otherwise (TB-SMA: the clamped switch makes the term continuous and exactly 0
 // beyond r_c) two of the five operations are contracted into FMAs.
-template <bool CANON>
+// DYN: the box edges are device state (a barostat is or was on); otherwise they are kernel parameters
+template <bool CANON, bool DYN = true>
 __device__ __forceinline__ double pair_r2(const double4 &pj, const double4 &pi, unsigned e, const DevSys &s,
                                           double &dx, double &dy, double &dz) {
   const unsigned code = e >> kIdxBits;
   if (code == 0) {
     dx = __dsub_rn(pj.x, pi.x); dy = __dsub_rn(pj.y, pi.y); dz = __dsub_rn(pj.z, pi.z);
   } else {
-    dx = image_delta(pj.x, pi.x, code & 3u, s.L[0]);
-    dy = image_delta(pj.y, pi.y, (code >> 2) & 3u, s.L[1]);
-    dz = image_delta(pj.z, pi.z, (code >> 4) & 3u, s.L[2]);
+    dx = image_delta(pj.x, pi.x, code & 3u, DYN ? s.st->box[0] : s.L0[0]);
+    dy = image_delta(pj.y, pi.y, (code >> 2) & 3u, DYN ? s.st->box[1] : s.L0[1]);
+    dz = image_delta(pj.z, pi.z, (code >> 4) & 3u, DYN ? s.st->box[2] : s.L0[2]);
   }
   if (CANON) return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
   return fma(dz, dz, fma(dy, dy, dx * dx));
@@ -372,7 +373,7 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
   }
 }
 
-template <int KIND, bool MULTI, bool FOLD>
+template <int KIND, bool MULTI, bool FOLD, bool DYN>
 __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s) {
   __shared__ double tab_sm[kExpTabLen];
   unsigned tab = 0;
@@ -392,7 +393,7 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
   auto prep = [&](unsigned e, const double4 &pj) {
     PairD d;
-    d.r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, d.dx, d.dy, d.dz);
+    d.r2 = pair_r2<KIND != MD_POT_TBSMA, DYN>(pj, pi, e, s, d.dx, d.dy, d.dz);
     d.w = pj.w; d.e = e;
     return d;
   };
@@ -562,7 +563,7 @@ __device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &
   }
 }
 
-template <int KIND, bool MULTI, bool OBS, bool FOLD>
+template <int KIND, bool MULTI, bool OBS, bool FOLD, bool DYN>
 __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
@@ -581,7 +582,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
   auto prep = [&](unsigned e, const double4 &pj) {
     PairD d;
-    d.r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, d.dx, d.dy, d.dz);
+    d.r2 = pair_r2<KIND != MD_POT_TBSMA, DYN>(pj, pi, e, s, d.dx, d.dy, d.dz);
     d.w = pj.w; d.e = e;
     return d;
   };
@@ -805,8 +806,14 @@ static void launch_density_k(md_system *sys, int grid) {
     else ++sys->launches, k_density_sub<KIND, false, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
     return;
   }
-  if (sys->d.nt > 1) ++sys->launches, k_density<KIND, true, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-  else ++sys->launches, k_density<KIND, false, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  ++sys->launches;
+  if (sys->d.dyn_box) {
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    else k_density<KIND, false, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  } else {
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    else k_density<KIND, false, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  }
 }
 
 int launch_density(md_system *sys) {
@@ -835,11 +842,21 @@ static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams 
     return;
   }
   if (multi) {
-    if (obs) k_force<KIND, true, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-    else k_force<KIND, true, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    if (sys->d.dyn_box) {
+      if (obs) k_force<KIND, true, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force<KIND, true, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    } else {
+      if (obs) k_force<KIND, true, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force<KIND, true, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    }
   } else {
-    if (obs) k_force<KIND, false, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-    else k_force<KIND, false, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    if (sys->d.dyn_box) {
+      if (obs) k_force<KIND, false, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force<KIND, false, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    } else {
+      if (obs) k_force<KIND, false, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      else k_force<KIND, false, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+    }
   }
 }
 

@@ -108,6 +108,44 @@ int launch_ekin(md_system *sys) {
   return (int)cudaGetLastError();
 }
 
+// ---- Berendsen barostat, eq.(5)-(6) ---------------------------------------------------
+// P = (2/3 E_kin + 1/3 tr W) / V of box 0 (one box only); dt_over_tau < 0: pressure only, no scaling.
+__global__ void k_pressure_mu(const __grid_constant__ DevSys s, double dt_over_tau, double P0) {
+  DevState *st = s.st;
+  const double trw = (s.box_virial[0] + s.box_virial[1]) + s.box_virial[2];
+  const double V = st->box[0] * st->box[1] * st->box[2];
+  const double P = ((2.0 / 3.0) * s.box_ekin[0] + trw / 3.0) / V;
+  st->pressure = P;
+  if (dt_over_tau < 0.0) return;
+  const double mu = cbrt(1.0 - dt_over_tau * (P0 - P));
+  st->mu = mu;
+  st->box[0] *= mu; st->box[1] *= mu; st->box[2] *= mu;
+}
+
+__global__ void __launch_bounds__(256) k_scale_positions(const __grid_constant__ DevSys s) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const double mu = s.st->mu;
+  double4 p = s.pos[i];
+  p.x *= mu; p.y *= mu; p.z *= mu;
+  s.pos[i] = p;
+}
+
+int launch_pressure(md_system *sys) {
+  if (launch_ekin(sys) != 0) return 1;
+  ProfScope p(sys, MD_K_REDUCE);
+  ++sys->launches, k_pressure_mu<<<1, 1, 0, sys->stream>>>(sys->d, -1.0, 0.0);
+  return (int)cudaGetLastError();
+}
+
+int launch_barostat(md_system *sys, double dt) {
+  if (launch_ekin(sys) != 0) return 1;
+  ProfScope p(sys, MD_K_INTEGRATE);
+  ++sys->launches, k_pressure_mu<<<1, 1, 0, sys->stream>>>(sys->d, dt / sys->baro_tau, sys->baro_P0);
+  ++sys->launches, k_scale_positions<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d);
+  return (int)cudaGetLastError();
+}
+
 // ---- FP64 issue-rate diagnostic: 8 independent DFMA chains per thread, register resident ---------
 __global__ void __launch_bounds__(256) k_dfma_chains(double *out, int iters, double a, double b, long long *clocks) {
   double x0 = threadIdx.x * 1e-3, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0,

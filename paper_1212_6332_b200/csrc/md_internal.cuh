@@ -27,6 +27,8 @@ struct DevState {
   int max_neighbors;               // of the last build
   unsigned long long rebuilds;
   unsigned long long list_entries; // sum of list lengths of the last build
+  double box[3];                   // CURRENT box edges (md_create's, then scaled by the barostat): every kernel reads them here
+  double mu, pressure;             // last barostat step
   unsigned long long graph_body_runs; // rebuild bodies that ran inside a CUDA-graph step (for the launch count)
 };
 
@@ -57,10 +59,10 @@ struct TableParams {
 // Everything a kernel needs, passed by value as a __grid_constant__ parameter.
 struct DevSys {
   int N, nb, npb, nt;
-  double L[3], hL[3];
+  double rl;                       // cutoff + skin
+  double L0[3]; int dyn_box;       // box edges: L0 while no barostat has touched them, else DevState::box (box_edge())
   double rc2, rl2, thr2, rin2;     // rin2: build-time split of a list row (pairs with r2 < rin2 first)
   int nc[3], tnc, ncell;           // cells per box (per dim, total) and cells of all boxes
-  double cell_scale[3];            // nc/L
   int cap;                         // neighbour capacity per atom
   int tiles_per_box;               // 32-atom tiles per box
   int kind;
@@ -91,6 +93,9 @@ struct DevSys {
 __host__ __device__ inline size_t nbr_row_offset(size_t tile, int cap, int lane) { return (tile * (size_t)(cap >> 2) * 32 + lane) * 4; }
 __host__ __device__ inline size_t nbr_entry(int k) { return (size_t)(k >> 2) * 128 + (k & 3); }
 
+// current box edge a: a kernel parameter until a barostat is switched on, device state from then on
+__device__ __forceinline__ double box_edge(const DevSys &s, int a) { return s.dyn_box ? s.st->box[a] : s.L0[a]; }
+
 struct ProfClass { std::vector<cudaEvent_t> ev; size_t used = 0; long dropped = 0; };
 
 }  // namespace md
@@ -101,6 +106,7 @@ struct md_system {
   double mass_ev[MD_MAX_TYPES];    // eV fs^2 / A^2
   double cutoff, skin;
   double thermo_Te, thermo_tau;    // eq.(4) thermostat; tau <= 0: off
+  double baro_P0, baro_tau;        // eq.(5) barostat; tau <= 0: off
   bool have_list, forces_valid, observables_valid;
   bool opt_step_obs, opt_profile, opt_graph;
   // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
@@ -145,6 +151,8 @@ int launch_force(md_system *s, bool observables, double half_dt); // half_dt = d
 int launch_kick_drift(md_system *s, double dt);
 int launch_reduce_boxes(md_system *s);
 int launch_ekin(md_system *s);
+int launch_barostat(md_system *s, double dt);                 // ekin, mu and box update, scale positions (end of a step)
+int launch_pressure(md_system *s);                            // ekin + eq.(6) into DevState::pressure
 
 struct ProfScope {                 // brackets launches of one kernel class with events when profiling is on
   md_system *s; int cls; cudaEvent_t stop = nullptr;

@@ -32,7 +32,11 @@ __global__ void k_decide(const __grid_constant__ DevSys s, unsigned long long th
   st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
   st->maxd2_bits = 0ull;
   st->force_rebuild = 0;
-  if (go) { st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1; }
+  if (go) {
+    st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1;
+    for (int a = 0; a < 3; ++a)                        // the cell grid is fixed at md_create; a barostat may have shrunk the box
+      if (!(box_edge(s, a) >= s.nc[a] * s.rl)) st->error_flags |= MD_FLAG_BOX;
+  }
   if (use_cond) { cudaGraphSetConditional(cond, go ? 1u : 0u); if (go) st->graph_body_runs += 1; }
 }
 
@@ -51,13 +55,14 @@ __global__ void k_bin(const __grid_constant__ DevSys s) {
     atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
     p.x = p.y = p.z = 0.0;
   }
-  p.x = wrap_coord(p.x, s.L[0]);
-  p.y = wrap_coord(p.y, s.L[1]);
-  p.z = wrap_coord(p.z, s.L[2]);
+  const double L0 = box_edge(s, 0), L1 = box_edge(s, 1), L2 = box_edge(s, 2);
+  p.x = wrap_coord(p.x, L0);
+  p.y = wrap_coord(p.y, L1);
+  p.z = wrap_coord(p.z, L2);
   s.pos[i] = p;
-  const int cx = cell_coord(p.x, s.cell_scale[0], s.nc[0]);
-  const int cy = cell_coord(p.y, s.cell_scale[1], s.nc[1]);
-  const int cz = cell_coord(p.z, s.cell_scale[2], s.nc[2]);
+  const int cx = cell_coord(p.x, s.nc[0] / L0, s.nc[0]);
+  const int cy = cell_coord(p.y, s.nc[1] / L1, s.nc[1]);
+  const int cz = cell_coord(p.z, s.nc[2] / L2, s.nc[2]);
   // multiple boxes: cell ids of box I shifted by I*TNC
   const int cid = (i / s.npb) * s.tnc + (cx * s.nc[1] + cy) * s.nc[2] + cz;
   s.cell_id[i] = cid;
@@ -208,9 +213,10 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   const size_t tile = (size_t)box * s.tiles_per_box + (local >> 5);
   unsigned *row = s.nbr + nbr_row_offset(tile, s.cap, local & 31);
   const double4 pi = s.pos[i];
-  const int cx = cell_coord(pi.x, s.cell_scale[0], s.nc[0]);
-  const int cy = cell_coord(pi.y, s.cell_scale[1], s.nc[1]);
-  const int cz = cell_coord(pi.z, s.cell_scale[2], s.nc[2]);
+  const double L[3] = {box_edge(s, 0), box_edge(s, 1), box_edge(s, 2)};
+  const int cx = cell_coord(pi.x, s.nc[0] / L[0], s.nc[0]);
+  const int cy = cell_coord(pi.y, s.nc[1] / L[1], s.nc[1]);
+  const int cz = cell_coord(pi.z, s.nc[2] / L[2], s.nc[2]);
   const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
   const int zlo = max(cz - 1, 0), zhi = min(cz + 1, ncz - 1);
   int n_all = 0;
@@ -243,19 +249,19 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   for (int ox = -1; ox <= 1; ++ox) {
     int jx = cx + ox;
     double sx = 0.0; unsigned kx = 0;
-    if (jx < 0) { jx += ncx; sx = -s.L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = s.L[0]; kx = 1; }
+    if (jx < 0) { jx += ncx; sx = -L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = L[0]; kx = 1; }
     for (int oy = -1; oy <= 1; ++oy) {
       int jy = cy + oy;
       double sy = 0.0; unsigned ky = 0;
-      if (jy < 0) { jy += ncy; sy = -s.L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = s.L[1]; ky = 1; }
+      if (jy < 0) { jy += ncy; sy = -L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = L[1]; ky = 1; }
       const int col = box * s.tnc + (jx * ncy + jy) * ncz;
       // up to three runs: the in-range z cells, plus the wrapped cell on either side
       for (int run = 0; run < 3; ++run) {
         int c0, c1;
         double sz = 0.0; unsigned kz = 0;
         if (run == 0) { c0 = col + zlo; c1 = col + zhi; }
-        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; sz = -s.L[2]; kz = 2; }
-        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; sz = s.L[2]; kz = 1; }
+        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; sz = -L[2]; kz = 2; }
+        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; sz = L[2]; kz = 1; }
         const int jbeg = s.cell_start[c0], jend = s.cell_start[c1 + 1];
         if (PERCELL) {
           // four candidates per trip: the four loads are issued together (read-only path, so the list stores
@@ -282,9 +288,9 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           for (int j = jbeg; j < jend; ++j) {
             const double4 pj = s.pos[j];
             unsigned ax, ay, az;
-            const double dx = min_image(__dsub_rn(pj.x, pi.x), s.L[0], s.hL[0], ax);
-            const double dy = min_image(__dsub_rn(pj.y, pi.y), s.L[1], s.hL[1], ay);
-            const double dz = min_image(__dsub_rn(pj.z, pi.z), s.L[2], s.hL[2], az);
+            const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
+            const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
+            const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
             const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
             if (r2 < s.rl2 && j != i) keep(j, r2, ax | (ay << 2) | (az << 4));
           }

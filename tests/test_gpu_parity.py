@@ -209,6 +209,65 @@ def test_thermostat_trajectory(md, case, variant):
         g.set_thermostat(-1.0, 10.0)
 
 
+@pytest.mark.parametrize("case,graph", [("cfg0", 1), ("cfg3a_small", 1), ("alloy_tables", 0), ("noncubic", 1)])
+def test_barostat_trajectory(md, case, graph):
+    """eq.(5)-(6) Berendsen barostat (row f1): box, coordinates and pressure follow the oracle's, step by step."""
+    w = CASES[case]()
+    if case == "noncubic":
+        w.positions = w.positions - np.array([40.0, -33.0, 1000.0])      # scaling acts on the coordinates as given
+    o = oracle_of(w)
+    g = md.MDSystem(w)
+    g.set_option(md.MD_OPT_GRAPH, graph)
+    assert abs(g.pressure() - o.pressure()) <= 1e-12 * abs(o.pressure())
+    P0 = 0.0 if w.pot_kind == 0 else o.pressure()        # the synthetic Fe-form EAM sits at -33 GPa: hold it there
+    for x in (o, g):
+        x.set_barostat(P0, 15.0)
+        x.set_thermostat(500.0, 100.0)
+    for n in (1, 59):
+        o.step(n, w.dt)
+        g.step(n, w.dt)
+    assert np.abs(g.box() / o.box() - 1.0).max() <= 1e-13
+    assert np.abs(g.box() / w.box - 1.0).max() > 1e-5     # the box did move
+    d = g.positions() - o.positions()
+    d -= np.round(d / o.box()) * o.box()
+    assert np.abs(d).max() <= X_TOL
+    assert abs(g.pressure() - o.pressure()) <= 1e-10 * max(abs(o.pressure()), 1e-3)
+    gep, gek = g.energies()
+    oep, oek = o.energies()
+    assert abs(gep.sum() - oep.sum()) <= 1e-11 * abs(oep.sum()) and abs(gek.sum() - oek.sum()) <= 1e-10 * oek.sum()
+    assert g.stats()["error_flags"] == 0
+    # the list the device holds is the oracle's list for the device's positions and box
+    g.build_neighbors()
+    w2 = CASES[case]()
+    w2.box = g.box()
+    o2 = oracle_of(w2, positions=g.positions())
+    o2.build_neighbors()
+    assert np.array_equal(g.neighbors(192)[1], o2.neighbors(192)[1])
+
+
+def test_barostat_relaxes_perfect_lattice_to_closed_form_and_guards(md):
+    """P0 = 0 on a perfect Cu lattice at rest: the box converges to the minimum of the closed-form E(a)
+    (tests/golden/lattice_pins.txt cu49.a_eq, mpmath), on the device as in the oracle."""
+    pins = dict(l.split(" = ") for l in open(__import__("os").path.join(__import__("os").path.dirname(__file__), "golden", "lattice_pins.txt"))
+                if " = " in l)
+    w = workloads.cu_fcc(6, sigma=0.0, temperature=0.0)
+    w.velocities = np.zeros_like(w.velocities)
+    g = md.MDSystem(w)
+    g.set_barostat(0.0, 1.75)
+    g.step(80, 1.0)
+    assert abs(g.box()[0] / 6 - float(pins["cu49.a_eq"])) < 1e-9 and abs(g.pressure()) < 1e-11
+    assert abs(g.energies()[0].sum() / w.n_atoms - float(pins["cu49.E_eq"])) < 1e-12
+    # a huge external pressure shrinks the cells below cutoff + skin: sticky flag, MD_EBOX
+    g = md.MDSystem(workloads.config(0))
+    g.set_barostat(5.0, 20.0)
+    with pytest.raises(md.MDError) as ei:
+        g.step(40, 1.0)
+        g.stats(); g.positions()
+    assert ei.value.code == md.MD_EBOX
+    with pytest.raises(md.MDError):
+        md.MDSystem(workloads.config(2, scale=2)).set_barostat(0.0, 5.0)
+
+
 def test_run_to_run_determinism(md):
     w = CASES["cfg2_small"]()
     res = []

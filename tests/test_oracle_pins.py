@@ -580,3 +580,51 @@ def test_thermostat_off_limits_and_crystal_temperature():
     kw, _ = _free_atoms(np.array([0.0, 0.002]))
     o = Oracle(**kw); o.set_thermostat(300.0, 50.0); o.step(5, 1.0)
     assert np.all(o.velocities()[0] == 0.0) and np.all(np.isfinite(o.velocities()))
+
+
+# ---------------------------------------------------------------- Berendsen barostat, eq.(5)-(6)
+def test_pressure_closed_forms(pins):
+    """eq.(6): the virial part on a perfect lattice (= -dE/dV from the lattice-sum pin) and the ideal-gas part"""
+    w = perfect_cu(6)
+    o = Oracle(w, velocities=np.zeros_like(w.velocities))
+    a = 3.615
+    assert abs(o.pressure() - 4 * pins["cu49.W"] / (3 * a ** 3)) < 1e-15          # N W_i / (3 V), 4 atoms per a^3
+    assert abs(o.pressure() * 160.21766208 - 0.66154) < 1e-4                        # GPa, SURVEY.md section 8(c)
+    kw, types = _free_atoms(np.array([0.003, 0.004, 0.002, 0.005]))
+    m = np.array(kw["mass"])[types] * AMU
+    ek = 0.5 * (m * np.array([0.003, 0.004, 0.002, 0.005]) ** 2).sum()
+    assert abs(Oracle(**kw).pressure() - (2.0 / 3.0) * ek / 39.0 ** 3) < 1e-20      # no forces: P V = N k_B T = 2/3 E_kin
+
+
+def test_barostat_one_step_formula_and_relaxation_to_the_pinned_lattice_constant(pins):
+    w = perfect_cu(6)
+    v0 = np.zeros_like(w.velocities)
+    # one step, atoms at rest on the perfect lattice: mu = cbrt(1 - dt/tau (P0 - P)) exactly, box and coordinates scaled
+    o = Oracle(w, velocities=v0)
+    P, P0, tau, dt = o.pressure(), -0.002, 5.0, 1.0
+    o.set_barostat(P0, tau)
+    x0 = o.positions()
+    o.step(1, dt)
+    mu = np.cbrt(1.0 - dt / tau * (P0 - P))
+    assert mu > 1.0                                                                # P > P0: the box grows
+    assert np.abs(o.box() / w.box - mu).max() < 1e-15 and np.abs(o.positions() - mu * x0).max() < 1e-12
+    # P0 = 0: the box relaxes to the minimum of the closed-form E(a): the pinned equilibrium lattice constant
+    o = Oracle(w, velocities=v0)
+    o.set_barostat(0.0, 1.75)                                                       # dt/tau ~ 0.5/B, B ~ 0.87 eV/A^3
+    o.step(80, 1.0)
+    assert abs(o.box()[0] / 6 - pins["cu49.a_eq"]) < 1e-9
+    assert abs(o.pressure()) < 1e-12 and np.abs(o.compute_forces()[0]).max() < 1e-10
+    assert abs(o.energies()[0].sum() / w.n_atoms - pins["cu49.E_eq"]) < 1e-12
+    # off by default / tau <= 0; refuses batched boxes
+    a, b = Oracle(workloads.config(0)), Oracle(workloads.config(0))
+    b.set_barostat(0.0, 0.0)
+    a.step(10, 1.0); b.step(10, 1.0)
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(b.box(), workloads.config(0).box)
+    with pytest.raises(OracleError):
+        Oracle(workloads.config(2, scale=2)).set_barostat(0.0, 5.0)
+    # thermal run under pressure control keeps the list valid (x_ref is not scaled: the rebuild rule sees the scaling)
+    o = Oracle(workloads.config(0))
+    o.set_barostat(0.0, 20.0)
+    for _ in range(8):
+        o.step(10, 1.0)
+        assert o.list_covers_cutoff()
