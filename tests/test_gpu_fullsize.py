@@ -73,3 +73,27 @@ def test_full_size(md, cfg, nsteps, stride):
     assert abs(sg["rebuilds"] - so["rebuilds"]) <= 1
     if cfg == "4":
         assert sg["rebuilds"] >= nsteps // 3     # the cascade does stress the rebuild rate
+
+
+def test_sixteen_million_atoms(md):
+    """north_star: one B200's memory holds multi-million-atom systems directly.  Cu fcc 160^3 = 16,384,000 atoms
+    (workspace ~10 GB): every force component and the per-atom energies against the oracle, then a few steps."""
+    from oracle import Oracle
+    w = workloads.config("3a", scale=160)
+    assert w.n_atoms == 16_384_000
+    o, g = Oracle(w), md.MDSystem(w)
+    of, oe, ow = o.compute_forces()
+    gf, ge, gw = g.compute_forces()
+    assert np.abs(gf - of).max() <= F_TOL
+    assert np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    assert abs(ge.sum() - oe.sum()) <= E_REL * abs(oe.sum())
+    assert np.abs(gw - ow).max() <= 1e-11 * np.abs(ow).max()
+    st = g.stats()
+    assert st["error_flags"] == 0 and st["max_neighbors"] == o.stats()["max_neighbors"]
+    assert st["list_entries"] == int(o.neighbors(stride=96)[0].sum())          # same number of listed pairs
+    del of, gf, oe, ge
+    o.step(3, w.dt)
+    g.step(3, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
