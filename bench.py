@@ -165,6 +165,19 @@ def time_oracle(workload: str, budget_s: float) -> dict:
             "ms_per_step": 1e3 * t / n}
 
 
+def whole_job_value(ms_local: float, n_atoms_per_rank: int, steps: int, world: int, device: str = "cuda") -> tuple[float, float]:
+    """Replicas only: every rank ran its own system for `steps` steps in `ms_local` ms of device
+    time; the job's time is the MAX over ranks and its value the atom-steps of ALL ranks over that time.  The one
+    collective of the whole benchmark (besides the barrier) is this all-reduce of a scalar."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return ms_max, world * n_atoms_per_rank * steps / (ms_max * 1e-3)
+
+
 def reference_arm(args, rank: int):
     if rank != 0:
         return
@@ -239,11 +252,7 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
         raise SystemExit(f"device error flags {st1['error_flags']}")
     launches = st1["kernel_launches"] - st0["kernel_launches"]
     rebuilds = st1["rebuilds"] - st0["rebuilds"]
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * w.n_atoms * K / (ms_max * 1e-3)
+    ms_max, value = whole_job_value(ms, w.n_atoms, K, world)
 
     # ---- per-kernel device time over the same K steps, events around every launch (separate run) --------
     g.set_option(md.MD_OPT_PROFILE, 1)
