@@ -34,9 +34,9 @@ constexpr int kForceMinBlocks = MD_FORCE_MINB, kDensityMinBlocks = MD_DENS_MINB;
 
 // d = (x_j - x_i) with the image recorded at build time: code 0: none, 1: +L, 2: -L.
 __device__ __forceinline__ double image_delta(double xj, double xi, unsigned code, double L) {
-  double d = __dsub_rn(xj, xi);
-  if (code) d = (code == 2) ? __dsub_rn(d, L) : __dadd_rn(d, L);
-  return d;
+  // branch-free: d + (-L) is bit-identical to d - L and d + 0.0 to d (up to the sign of a zero)
+  const double shift = (code & 1u) ? L : ((code & 2u) ? -L : 0.0);
+  return __dadd_rn(__dsub_rn(xj, xi), shift);
 }
 
 // CANON: r2 = (dx*dx + dy*dy) + dz*dz with every operation rounded once (reading A3), needed where r2 < rc2 decides a

@@ -285,14 +285,28 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
             test_keep(j, r2, code);
           }
         } else {
-          for (int j = jbeg; j < jend; ++j) {
-            const double4 pj = s.pos[j];
+          // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
+          auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
             unsigned ax, ay, az;
             const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
             const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
             const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            if (r2 < s.rl2 && j != i) keep(j, r2, ax | (ay << 2) | (az << 4));
+            r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            code = ax | (ay << 2) | (az << 4);
+          };
+          int j = jbeg;
+          for (; j + 4 <= jend; j += 4) {
+            const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
+            double r0, r1, r2, r3;
+            unsigned c0, c1, c2, c3;
+            dist2m(p0, r0, c0); dist2m(p1, r1, c1); dist2m(p2, r2, c2); dist2m(p3, r3, c3);
+            test_keep(j, r0, c0); test_keep(j + 1, r1, c1); test_keep(j + 2, r2, c2); test_keep(j + 3, r3, c3);
+          }
+          for (; j < jend; ++j) {
+            double r2;
+            unsigned c;
+            dist2m(ld_pos(s.pos + j), r2, c);
+            test_keep(j, r2, c);
           }
         }
       }
