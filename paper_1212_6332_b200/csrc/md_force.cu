@@ -330,9 +330,14 @@ __device__ __forceinline__ AtomRow atom_row(const DevSys &s, int box, int local,
 }
 
 __device__ __forceinline__ unsigned stage_exp_table(const DevSys &s, double *tab) {
-  if (threadIdx.x < kExpTabLen) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
+  if (threadIdx.x < kExpTabLen - 1) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
+  const unsigned a = (unsigned)__cvta_generic_to_shared(tab);
+  if (threadIdx.x == kExpTabLen - 1) reinterpret_cast<unsigned *>(tab + (kExpTabLen - 1))[0] = a;   // the last slot is free
   __syncthreads();
-  return (unsigned)__cvta_generic_to_shared(tab);
+  // read the address back through an opaque load: ptxas would otherwise recompute it (S2UR + ULEA + MOV) at every use
+  unsigned t;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(t) : "r"(a + 8u * (kExpTabLen - 1)));
+  return t;
 }
 
 // ------------------------------------------------------------------------------------------------
