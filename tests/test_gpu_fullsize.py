@@ -97,3 +97,22 @@ def test_sixteen_million_atoms(md):
     d = g.positions() - o.positions()
     d -= np.round(d / w.box) * w.box
     assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+
+
+def test_thermostat_and_barostat_at_full_size(md):
+    """rows f1a/f1b on the bench workload: 1,048,576 Cu atoms, eq.(4) bath at 600 K and eq.(5) pressure control at P0 = 0."""
+    from oracle import Oracle
+    w = workloads.config("3a")
+    o, g = Oracle(w), md.MDSystem(w)
+    for x in (o, g):
+        x.set_thermostat(600.0, 80.0)
+        x.set_barostat(0.0, 20.0)
+    o.step(30, w.dt)
+    g.step(30, w.dt)
+    assert np.abs(g.box() / o.box() - 1.0).max() <= 1e-13 and np.abs(g.box() / w.box - 1.0).max() > 1e-6
+    d = g.positions() - o.positions()
+    d -= np.round(d / o.box()) * o.box()
+    assert np.abs(d).max() <= X_TOL
+    assert np.abs(g.velocities() - o.velocities()).max() <= 1e-9
+    assert abs(g.pressure() - o.pressure()) <= 1e-10 * max(abs(o.pressure()), 1e-3)
+    assert g.stats()["error_flags"] == 0
