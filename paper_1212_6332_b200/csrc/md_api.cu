@@ -263,10 +263,7 @@ static int deliver(md_system *s, void *user, const void *dev, size_t bytes, bool
 }
 
 static int forces_sequence(md_system *s, bool observables, double half_dt) {
-  int rc;
-  if ((rc = launch_rebuild_chain(s)) != 0) return MD_ECUDA;
-  if ((rc = launch_density(s)) != 0) return MD_ECUDA;
-  if ((rc = launch_force(s, observables, half_dt)) != 0) return MD_ECUDA;
+  if (launch_rebuild_chain(s) != 0 || launch_density(s) != 0 || launch_force(s, observables, half_dt) != 0) return MD_ECUDA;
   s->have_list = true;
   s->forces_valid = true;
   s->observables_valid = observables;
@@ -426,7 +423,6 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   o.rl = rl; o.dyn_box = 0;
   o.rc2 = d->cutoff * d->cutoff; o.rin2 = o.rc2; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
   o.tnc = g.tnc; o.ncell = g.ncell; o.cap = g.cap; o.tiles_per_box = g.tiles_per_box;
-  s->n_force_blocks = g.n_blocks;
   for (int t = 0; t < d->n_types; ++t) s->mass_ev[t] = d->mass[t] * kAmuToEvFs2PerA2;
   const size_t N = (size_t)o.N, nt2 = (size_t)o.nt * o.nt;
   cudaStream_t st = s->stream;

@@ -115,7 +115,6 @@ struct md_system {
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
-  int n_force_blocks;
   md::ProfClass prof[MD_K_COUNT];
 };
 
@@ -149,7 +148,6 @@ int launch_density(md_system *s);
 int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
 int launch_force(md_system *s, bool observables, double half_dt); // half_dt = dt/2 (0: no velocity update)
 int launch_kick_drift(md_system *s, double dt);
-int launch_reduce_boxes(md_system *s);
 int launch_ekin(md_system *s);
 int launch_barostat(md_system *s, double dt);                 // ekin, mu and box update, scale positions (end of a step)
 int launch_pressure(md_system *s);                            // ekin + eq.(6) into DevState::pressure
