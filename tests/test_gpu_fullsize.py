@@ -116,3 +116,35 @@ def test_thermostat_and_barostat_at_full_size(md):
     assert np.abs(g.velocities() - o.velocities()).max() <= 1e-9
     assert abs(g.pressure() - o.pressure()) <= 1e-10 * max(abs(o.pressure()), 1e-3)
     assert g.stats()["error_flags"] == 0
+
+
+def test_maximum_atom_count(md):
+    """The largest system the list entry format admits: 2^26 = 67,108,864 atoms (Cu fcc 256^3, 26-bit slot index).
+    Too large for a full oracle run inside the test budget, so: properties that hold at any size, and element-wise
+    parity on a cut-out.  The force on an atom depends on atoms within 2 r_c (its neighbours and their densities),
+    so inside a 44 A cube cut out of the big system, atoms further than 2 r_c from the cube's faces feel exactly
+    the forces of the full system; the oracle evaluates the cut-out as a cluster in vacuum."""
+    from oracle import Oracle
+    w = workloads.config("3a", scale=256)
+    assert w.n_atoms == 1 << 26
+    g = md.MDSystem(w)
+    f, e, vir = g.compute_forces()
+    st = g.stats()
+    assert st["error_flags"] == 0 and 49 <= st["max_neighbors"] <= 60
+    assert abs(st["list_entries"] / w.n_atoms - 52.7) < 0.1          # 42 in-cutoff + 89 % of the 12 atoms of the 5.112 A shell
+    assert np.abs(f.sum(0)).max() < 1e-6                                       # Newton's third law over 3.5e9 directed pairs
+    assert abs(e.sum() / w.n_atoms - (-3.4772)) < 2e-3                          # same ensemble as the smaller jittered crystals
+    lo, side, margin = np.array([300.0, 411.0, 520.0]), 44.0, 2 * 4.9 + 0.2
+    inside = np.all((w.positions >= lo) & (w.positions < lo + side), axis=1)
+    idx = np.nonzero(inside)[0]
+    cut = w.positions[idx] - lo + 30.0
+    o = Oracle(max_neighbors=96, pot_kind=0, mass=w.mass, tbsma=w.tbsma, box=np.full(3, side + 60.0), positions=cut, cutoff=w.cutoff, skin=w.skin,
+               velocities=np.zeros_like(cut), types=np.zeros(len(idx), np.int32), n_boxes=1)
+    of, oe, _ = o.compute_forces()
+    deep = np.all((cut >= 30.0 + margin) & (cut < 30.0 + side - margin), axis=1)
+    assert deep.sum() > 1000
+    assert np.abs(f[idx][deep] - of[deep]).max() <= F_TOL
+    assert np.abs(e[idx][deep] - oe[deep]).max() <= 1e-12 * np.abs(oe).max()
+    del f, e
+    g.step(2, w.dt)
+    assert g.stats()["error_flags"] == 0 and g.stats()["steps"] == 2
