@@ -268,6 +268,25 @@ def test_barostat_relaxes_perfect_lattice_to_closed_form_and_guards(md):
         md.MDSystem(workloads.config(2, scale=2)).set_barostat(0.0, 5.0)
 
 
+def test_two_systems_interleaved_and_profile_toggle(md):
+    """every system owns its step graph and conditional handle; MD_OPT_PROFILE switches to plain launches and back"""
+    w1, w2 = CASES["cfg0"](), CASES["cfg3a_small"]()
+    a, b, ra, rb = md.MDSystem(w1), md.MDSystem(w2), md.MDSystem(w1), md.MDSystem(w2)
+    for n in (3, 17, 30):
+        a.step(n, 1.0)
+        b.step(n, 1.0)
+    ra.step(50, 1.0)
+    rb.step(50, 1.0)
+    assert np.array_equal(a.positions(), ra.positions()) and np.array_equal(b.positions(), rb.positions())
+    a.set_option(md.MD_OPT_PROFILE, 1)
+    a.step(5, 1.0)
+    assert a.profile()["force"][0] == 5
+    a.set_option(md.MD_OPT_PROFILE, 0)
+    a.step(5, 1.0)
+    ra.step(10, 1.0)
+    assert np.array_equal(a.positions(), ra.positions()) and a.stats()["error_flags"] == 0
+
+
 def test_run_to_run_determinism(md):
     w = CASES["cfg2_small"]()
     res = []
