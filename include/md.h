@@ -90,6 +90,11 @@ typedef struct {
   const double *F_val, *F_der;                     /* [n_types][nrho] */
   int max_neighbors;              /* list capacity per atom (the paper's MN); 0 = chosen from the number density */
   void *stream;                   /* cudaStream_t */
+  /* Optional per-pair cut-offs, the paper's RCUT(ity,jty), [n_types*n_types], HOST, symmetric,
+   * NULL = `cutoff` / `taper_on` for every pair.  pair_cutoff[ab] <= cutoff: a pair of types (a,b) contributes only
+   * for r < pair_cutoff[ab] (the list still holds every pair within cutoff + skin).  MD_POT_TBSMA: the switch of
+   * pair (a,b) runs from pair_taper_on[ab] (< pair_cutoff[ab]) to pair_cutoff[ab]. */
+  const double *pair_cutoff, *pair_taper_on;
 } md_desc;
 
 typedef struct {

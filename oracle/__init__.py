@@ -22,7 +22,7 @@ class _Desc(C.Structure):
                 ("mass", _D), ("pot_kind", C.c_int), ("A", _D), ("xi", _D), ("p", _D), ("q", _D), ("r0", _D),
                 ("taper_on", C.c_double), ("nr", C.c_int), ("dr", C.c_double), ("f_val", _D), ("f_der", _D),
                 ("phi_val", _D), ("phi_der", _D), ("nrho", C.c_int), ("drho", C.c_double), ("F_val", _D),
-                ("F_der", _D), ("max_neighbors", C.c_int)]
+                ("F_der", _D), ("max_neighbors", C.c_int), ("pair_cutoff", _D), ("pair_taper_on", _D)]
 
 
 class _Stats(C.Structure):
@@ -119,6 +119,12 @@ class Oracle:
             d.nr, d.dr, d.nrho, d.drho = int(tab["nr"]), float(tab["dr"]), int(tab["nrho"]), float(tab["drho"])
             for k in ("f_val", "f_der", "phi_val", "phi_der", "F_val", "F_der"):
                 a = _f64(tab[k])
+                self._keep.append(a)
+                setattr(d, k, _dp(a))
+        for k in ("pair_cutoff", "pair_taper_on"):
+            v = g(k)
+            if v is not None:
+                a = _f64(v)
                 self._keep.append(a)
                 setattr(d, k, _dp(a))
         d.max_neighbors = int(max_neighbors)

@@ -33,6 +33,7 @@ struct oracle_system {
   int *type;
   int kind;
   double *A, *xi, *p, *q, *r0, r_on;     /* [nt*nt] */
+  double *rc_p, *rc2_p, *ron_p;          /* per type pair: cut-off, its square, taper start (RCUT(ity,jty)) */
   int nr, nrho; double dr, drho;
   double *f_val, *f_der, *phi_val, *phi_der, *F_val, *F_der;
   int stride, *ncount, *nlist, have_list, forces_valid;
@@ -142,7 +143,7 @@ static void radial(const oracle_system *s, int ti, int tj, double r, double *f, 
   int tp = ti * s->nt + tj;
   if (s->kind == 0) {
     double o[6];
-    oracle_tbsma_eval(r, s->A[tp], s->xi[tp], s->p[tp], s->q[tp], s->r0[tp], s->r_on, s->rc, o);
+    oracle_tbsma_eval(r, s->A[tp], s->xi[tp], s->p[tp], s->q[tp], s->r0[tp], s->ron_p[tp], s->rc_p[tp], o);
     *f = o[0]; *df = o[1]; *V = o[2]; *dV = o[3];
   } else {
     size_t off = (size_t)tp * s->nr;
@@ -176,6 +177,16 @@ int oracle_create(const oracle_desc *d, oracle_system **out) {
   s->m = dup_d(d->mass, s->nt);
   for (int t = 0; t < s->nt; ++t) { if (!(s->m[t] > 0.0)) { oracle_destroy(s); return ORACLE_EINVAL; } s->m[t] *= AMU_EV; }
   s->kind = d->pot_kind;
+  /* per-pair cut-offs (RCUT(ity,jty)); default: the global ones */
+  s->rc_p = dup_d(NULL, nt2); s->rc2_p = dup_d(NULL, nt2); s->ron_p = dup_d(NULL, nt2);
+  for (int a = 0; a < s->nt; ++a)
+    for (int b = 0; b < s->nt; ++b) {
+      const int k = a * s->nt + b, kt = b * s->nt + a;
+      const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff, ron = d->pair_taper_on ? d->pair_taper_on[k] : d->taper_on;
+      if (!(rc > 0.0) || !(rc <= d->cutoff) || (d->pair_cutoff && d->pair_cutoff[kt] != rc) ||
+          (d->pot_kind == 0 && (!(ron < rc) || (d->pair_taper_on && d->pair_taper_on[kt] != ron)))) { oracle_destroy(s); return ORACLE_EINVAL; }
+      s->rc_p[k] = rc; s->rc2_p[k] = rc * rc; s->ron_p[k] = ron;
+    }
   if (s->kind == 0) {
     if (!d->A || !d->xi || !d->p || !d->q || !d->r0 || !(d->taper_on < d->cutoff)) { oracle_destroy(s); return ORACLE_EINVAL; }
     s->A = dup_d(d->A, nt2); s->xi = dup_d(d->xi, nt2); s->p = dup_d(d->p, nt2); s->q = dup_d(d->q, nt2);
@@ -208,6 +219,7 @@ int oracle_destroy(oracle_system *s) {
   free(s->x); free(s->v); free(s->f); free(s->xref); free(s->m); free(s->type);
   free(s->A); free(s->xi); free(s->p); free(s->q); free(s->r0);
   free(s->f_val); free(s->f_der); free(s->phi_val); free(s->phi_der); free(s->F_val); free(s->F_der);
+  free(s->rc_p); free(s->rc2_p); free(s->ron_p);
   free(s->ncount); free(s->nlist); free(s->rho); free(s->fp); free(s->eemb); free(s->eatom); free(s->wat);
   free(s->virial); free(s);
   return ORACLE_OK;
@@ -301,7 +313,7 @@ static int forces_internal(oracle_system *s) {
     for (int k = 0; k < s->ncount[i]; ++k) {
       int j = li[k];
       oracle_min_image(s->x + 3 * i, s->x + 3 * j, s->L, d, &r2);
-      if (r2 < s->rc2) {
+      if (r2 < s->rc2_p[s->type[i] * s->nt + s->type[j]]) {
         if (!(r2 > 0.0)) { bad |= 1; continue; }
         double r = sqrt(r2);
         radial(s, s->type[i], s->type[j], r, &f, &df, &V, &dV);
@@ -322,7 +334,7 @@ static int forces_internal(oracle_system *s) {
     for (int k = 0; k < s->ncount[i]; ++k) {
       int j = li[k];
       oracle_min_image(s->x + 3 * i, s->x + 3 * j, s->L, d, &r2);
-      if (r2 < s->rc2) {
+      if (r2 < s->rc2_p[s->type[i] * s->nt + s->type[j]]) {
         double r = sqrt(r2);
         radial(s, s->type[i], s->type[j], r, &f, &df, &V, &dV);
         double sij = dV + (s->fp[i] + s->fp[j]) * df;

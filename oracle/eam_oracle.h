@@ -48,6 +48,9 @@ typedef struct {
   int nrho; double drho;
   const double *F_val, *F_der;          /* [n_types][nrho] */
   int max_neighbors;                    /* list stride; 0 = choose */
+  /* optional per-pair cut-offs, the paper's RCUT(ity,jty): [n_types*n_types], symmetric,
+   * <= cutoff; NULL = cutoff / taper_on for every pair */
+  const double *pair_cutoff, *pair_taper_on;
 } oracle_desc;
 
 typedef struct { long steps, rebuilds; int max_neighbors, error_flags; double last_max_disp2; } oracle_stats;

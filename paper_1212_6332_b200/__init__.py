@@ -34,7 +34,8 @@ class MdDesc(C.Structure):
                 ("xi", C.c_void_p), ("p", C.c_void_p), ("q", C.c_void_p), ("r0", C.c_void_p), ("taper_on", C.c_double),
                 ("nr", C.c_int), ("dr", C.c_double), ("f_val", C.c_void_p), ("f_der", C.c_void_p),
                 ("phi_val", C.c_void_p), ("phi_der", C.c_void_p), ("nrho", C.c_int), ("drho", C.c_double),
-                ("F_val", C.c_void_p), ("F_der", C.c_void_p), ("max_neighbors", C.c_int), ("stream", C.c_void_p)]
+                ("F_val", C.c_void_p), ("F_der", C.c_void_p), ("max_neighbors", C.c_int), ("stream", C.c_void_p),
+                ("pair_cutoff", C.c_void_p), ("pair_taper_on", C.c_void_p)]
 
 
 class MdStats(C.Structure):
@@ -153,6 +154,12 @@ class MDSystem:
             d.nr, d.dr, d.nrho, d.drho = int(tab["nr"]), float(tab["dr"]), int(tab["nrho"]), float(tab["drho"])
             for k in ("f_val", "f_der", "phi_val", "phi_der", "F_val", "F_der"):
                 a = _host(tab[k], np.float64)
+                keep.append(a)
+                setattr(d, k, _ptr(a))
+        for k in ("pair_cutoff", "pair_taper_on"):                # optional per-pair cut-offs (RCUT(ity,jty))
+            v = g(k)
+            if v is not None:
+                a = np.ascontiguousarray(v, dtype=np.float64)
                 keep.append(a)
                 setattr(d, k, _ptr(a))
         d.max_neighbors = int(max_neighbors)

@@ -57,6 +57,16 @@ static int geometry(const md_desc *d, Geometry &g) {
   if (d->pot_kind == MD_POT_EAM_TABLE && (double)(d->nr - 1) * d->dr < d->cutoff * (1.0 - 1e-12)) return MD_EINVAL;
   if (d->pot_kind == MD_POT_TBSMA && !(d->taper_on < d->cutoff)) return MD_EINVAL;
   if (d->max_neighbors < 0) return MD_EINVAL;
+  for (int a = 0; a < d->n_types; ++a)
+    for (int b = 0; b < d->n_types; ++b) {
+      const int k = a * d->n_types + b, kt = b * d->n_types + a;
+      const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff;
+      if (!(rc > 0.0) || !(rc <= d->cutoff) || (d->pair_cutoff && d->pair_cutoff[kt] != rc)) return MD_EINVAL;
+      if (d->pot_kind == MD_POT_TBSMA) {
+        const double ron = d->pair_taper_on ? d->pair_taper_on[k] : d->taper_on;
+        if (!(ron < rc) || (d->pair_taper_on && d->pair_taper_on[kt] != ron)) return MD_EINVAL;
+      }
+    }
   const double rl = d->cutoff + d->skin;
   g.npb = d->n_atoms / d->n_boxes;
   double vol = 1.0;
@@ -421,6 +431,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     o.nc[a] = g.nc[a]; o.L0[a] = d->box[a];
   }
   o.rl = rl; o.dyn_box = 0;
+  for (int k = 0; k < o.nt * o.nt; ++k) { const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff; o.rc2p[k] = rc * rc; }
   o.rc2 = d->cutoff * d->cutoff; o.rin2 = o.rc2; o.rl2 = rl * rl; o.thr2 = (0.5 * d->skin) * (0.5 * d->skin);
   o.tnc = g.tnc; o.ncell = g.ncell; o.cap = g.cap; o.tiles_per_box = g.tiles_per_box;
   for (int t = 0; t < d->n_types; ++t) s->mass_ev[t] = d->mass[t] * kAmuToEvFs2PerA2;
@@ -454,10 +465,13 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
         delete s; return MD_EINVAL;
       }
     }
-    o.tb.inv_w = 1.0 / (d->cutoff - d->taper_on); o.tb.t0 = -d->taper_on * o.tb.inv_w; o.tb.m30_inv_w = -30.0 * o.tb.inv_w;
+    for (size_t k = 0; k < nt2; ++k) {
+      const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff, ron = d->pair_taper_on ? d->pair_taper_on[k] : d->taper_on;
+      o.tb.inv_w[k] = 1.0 / (rc - ron); o.tb.t0[k] = -ron * o.tb.inv_w[k]; o.tb.m30_inv_w[k] = -30.0 * o.tb.inv_w[k];
+    }
     // loop constants that the passes read from memory into registers (md_force.cu, LoopConsts)
     double *lc = s->exp_tab_host + 64;
-    lc[0] = 1.0 / 120.0; lc[1] = 0.375; lc[2] = 6.0; lc[3] = o.tb.inv_w; lc[4] = o.tb.bk_rho[0]; lc[5] = o.tb.bk_rep[0];
+    lc[0] = 1.0 / 120.0; lc[1] = 0.375; lc[2] = 6.0; lc[3] = o.tb.inv_w[0]; lc[4] = o.tb.bk_rho[0]; lc[5] = o.tb.bk_rep[0];
   } else {
     TableParams &t = o.tab;
     t.nr = d->nr; t.nrho = d->nrho; t.dr = d->dr; t.inv_dr = 1.0 / d->dr; t.drho = d->drho; t.inv_drho = 1.0 / d->drho;

@@ -348,7 +348,7 @@ __device__ __forceinline__ double density_term(const DevSys &s, const LoopConsts
   if (KIND == MD_POT_TBSMA) {
     const TbsmaParams &tb = s.tb;
     const double r = r2 * rsqrt_fast(r2, lc.c375);
-    const double S = switch_S(switch_t(r, lc.inv_w, tb.t0), lc.six);
+    const double S = switch_S(switch_t(r, MULTI ? tb.inv_w[tp] : lc.inv_w, tb.t0[tp]), lc.six);
     double e = exp_scaled(fma(-(MULTI ? tb.bk_rho[tp] : lc.bk_rho), r, tb.ak_rho[tp]), tab, lc.c5);
     if (!FOLD) e *= tb.pre_rho[tp];
     return e * S;
@@ -369,7 +369,7 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
 #pragma unroll
   MD_EACH r[q] = r2[q] * rinv[q];
 #pragma unroll
-  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0); }
+  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0[0]); }
   exp_scaled_n<NP>(xh, tab, lc.c5, eh);
 #pragma unroll
   MD_EACH {
@@ -404,7 +404,7 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   };
   auto term1 = [&](const PairD &d) {
     const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)d.w : 0, d.r2);
-    return (KIND == MD_POT_TBSMA || d.r2 < s.rc2) ? term : 0.0;
+    return (KIND == MD_POT_TBSMA || d.r2 < (MULTI ? s.rc2p[ti * s.nt + (int)d.w] : s.rc2)) ? term : 0.0;
   };
   walk_main(row.main, row.n_in, s.pos, zero, prep,
             [&](const PairD &a, const PairD &b) {
@@ -462,8 +462,8 @@ __device__ __forceinline__ void force_term(const DevSys &s, const LoopConsts &lc
   if (KIND == MD_POT_TBSMA) {
     const TbsmaParams &tb = s.tb;
     const double rinv = rsqrt_fast(r2, lc.c375), r = r2 * rinv;
-    const double t = switch_t(r, lc.inv_w, tb.t0);
-    const double S = switch_S(t, lc.six), dS = switch_dS(t, tb.m30_inv_w);
+    const double t = switch_t(r, MULTI ? tb.inv_w[tp] : lc.inv_w, tb.t0[tp]);
+    const double S = switch_S(t, lc.six), dS = switch_dS(t, tb.m30_inv_w[tp]);
     double eh = exp_scaled(fma(-(MULTI ? tb.bk_rho[tp] : lc.bk_rho), r, tb.ak_rho[tp]), tab, lc.c5);
     double er = exp_scaled(fma(-(MULTI ? tb.bk_rep[tp] : lc.bk_rep), r, tb.ak_rep[tp]), tab, lc.c5);
     if (!FOLD) { eh *= tb.pre_rho[tp]; er *= tb.pre_rep[tp]; }
@@ -494,11 +494,11 @@ __device__ __forceinline__ void force_term_n(const DevSys &s, const LoopConsts &
 #pragma unroll
   MD_EACH r[q] = r2[q] * rinv[q];
 #pragma unroll
-  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); xr[q] = fma(-lc.bk_rep, r[q], tb.ak_rep[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0); }
+  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); xr[q] = fma(-lc.bk_rep, r[q], tb.ak_rep[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0[0]); }
   exp_scaled_n<NP>(xh, tab, lc.c5, eh);
   exp_scaled_n<NP>(xr, tab, lc.c5, er);
 #pragma unroll
-  MD_EACH { S[q] = switch_S(t[q], lc.six); dS[q] = switch_dS(t[q], tb.m30_inv_w); }
+  MD_EACH { S[q] = switch_S(t[q], lc.six); dS[q] = switch_dS(t[q], tb.m30_inv_w[0]); }
 #pragma unroll
   MD_EACH {
     if (!FOLD) { eh[q] *= tb.pre_rho[0]; er[q] *= tb.pre_rep[0]; }
@@ -595,7 +595,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     double g, V = 0.0;
     const int tp = MULTI ? ti * s.nt + s.type[d.e & kIdxMask] : 0;
     force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, d.r2, pi.w + d.w, g, V);
-    if (KIND != MD_POT_TBSMA && !(d.r2 < s.rc2)) { g = 0.0; V = 0.0; }   // tables: strict cut-off, no switch (reading A9)
+    if (KIND != MD_POT_TBSMA && !(d.r2 < (MULTI ? s.rc2p[tp] : s.rc2))) { g = 0.0; V = 0.0; }   // tables: strict cut-off (A9)
     force_accumulate<OBS>(to, g, V, d.dx, d.dy, d.dz);
   };
   walk_main(row.main, row.n_in, s.posf, zero, prep,
@@ -687,8 +687,9 @@ __global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_consta
     double dx, dy, dz;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
     // main: TB-SMA is switched off continuously beyond r_c, tables need the strict test; skin: only pairs now inside r_c
-    if ((in_main && KIND == MD_POT_TBSMA) || r2 < s.rc2)
-      rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)pj.w : 0, r2);
+    const int tp = MULTI ? ti * s.nt + (int)pj.w : 0;
+    if ((in_main && KIND == MD_POT_TBSMA) || r2 < (MULTI && KIND != MD_POT_TBSMA ? s.rc2p[tp] : s.rc2))
+      rho += density_term<KIND, MULTI, FOLD>(s, lc, tab, tp, r2);
   });
 #pragma unroll
   for (int o = 1; o < kSub; o <<= 1) rho += __shfl_xor_sync(0xffffffffu, rho, o);
@@ -717,8 +718,8 @@ __global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant
     const double4 pj = gather32(s.posf + MD_GIDX(e));
     double dx, dy, dz, g, V = 0.0;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
-    if ((in_main && KIND == MD_POT_TBSMA) || r2 < s.rc2) {
-      const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
+    const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
+    if ((in_main && KIND == MD_POT_TBSMA) || r2 < (MULTI && KIND != MD_POT_TBSMA ? s.rc2p[tp] : s.rc2)) {
       force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, r2, pi.w + pj.w, g, V);
       force_accumulate<OBS>(acc, g, V, dx, dy, dz);
     }

@@ -38,8 +38,9 @@ struct TbsmaParams {               // per type pair, pre-combined on the host
   // ak_* = a_* 64/ln2 and bk_* = b_* 64/ln2: the exponent in units of ln2/64, as exp_scaled() takes it
   double ak_rho[kPairs], bk_rho[kPairs], b_rho[kPairs], pre_rho[kPairs];
   double ak_rep[kPairs], bk_rep[kPairs], b_rep[kPairs], pre_rep[kPairs];
-  double m30_inv_w;                // -30 inv_w (dS/dr prefactor)
-  double inv_w, t0;                // switch variable t = clamp(r inv_w + t0, 0, 1): inv_w = 1/(r_c - r_on), t0 = -r_on inv_w
+  // per type pair: switch variable t = clamp(r inv_w + t0, 0, 1), inv_w = 1/(r_c - r_on), t0 = -r_on inv_w;
+  // m30_inv_w = -30 inv_w (dS/dr prefactor)
+  double m30_inv_w[kPairs], inv_w[kPairs], t0[kPairs];
   int fold;
 };
 
@@ -61,6 +62,7 @@ struct DevSys {
   int N, nb, npb, nt;
   double rl;                       // cutoff + skin
   double L0[3]; int dyn_box;       // box edges: L0 while no barostat has touched them, else DevState::box (box_edge())
+  double rc2p[kPairs];             // per-pair cut-off squared (the paper's RCUT(ity,jty)); rc2 is their maximum
   double rc2, rl2, thr2, rin2;     // rin2: build-time split of a list row (pairs with r2 < rin2 first)
   int nc[3], tnc, ncell;           // cells per box (per dim, total) and cells of all boxes
   int cap;                         // neighbour capacity per atom

@@ -38,6 +38,9 @@ CASES = {
     "alloy_tbsma": lambda: workloads.alloy(workloads.config("3a", scale=10), 21),           # 4000 atoms
     "alloy_tbsma_boxes": lambda: workloads.alloy(workloads.config(2, scale=5), 22, 0.3),    # 5 boxes x 500, 30 % type 1
     "alloy_tables": lambda: workloads.alloy(workloads.config(1, scale=10), 23),             # 2000 atoms, 4 pair tables
+    # per-pair cut-offs, the paper's RCUT(ity,jty): r_c, 0.93 r_c, 0.97 r_c
+    "alloy_tbsma_rcut": lambda: workloads.alloy(workloads.config("3a", scale=10), 24, pair_cutoffs=True),
+    "alloy_tables_rcut": lambda: workloads.alloy(workloads.config(1, scale=10), 25, pair_cutoffs=True),
 }
 
 
@@ -94,7 +97,8 @@ def test_density_force_energy_virial(md, case):
 
 @pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 100), ("cfg1_small", 100), ("cfg2_small", 100),
                                          ("cfg3b_small", 40), ("cfg4_small", 100), ("alloy_tbsma", 100),
-                                         ("alloy_tbsma_boxes", 60), ("alloy_tables", 100)])
+                                         ("alloy_tbsma_boxes", 60), ("alloy_tables", 100), ("alloy_tbsma_rcut", 100),
+                                         ("alloy_tables_rcut", 100)])
 def test_trajectory(md, case, nsteps):
     w = CASES[case]()
     o = oracle_of(w)
@@ -134,7 +138,7 @@ def test_step_with_observables_matches_plain_step(md):
 
 @pytest.mark.parametrize("variant", [1, 2])
 @pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small", "alloy_tbsma",
-                                  "alloy_tables"])
+                                  "alloy_tables", "alloy_tbsma_rcut", "alloy_tables_rcut"])
 def test_both_pass_variants(md, case, variant):
     """One thread per atom (what large systems run) and 8 lanes per atom (small systems), forced on the same input."""
     w = CASES[case]()

@@ -436,9 +436,9 @@ def test_isolated_atom_and_empty_neighbourhood():
 
 
 # ---------------------------------------------------------------- binary alloys (PAPER.md:78 rho^(ab), V^(ab))
-def _alloy_energy_numpy(pos, types, tb, cutoff):
+def _alloy_energy_numpy(pos, types, tb, cutoff, pair_cutoff=None, pair_taper_on=None):
     """eq.(1) with type-pair parameters written out in numpy (direct double loop, float64); index [ti*2 + tj]."""
-    ron = tb["taper_on"]
+    ron0 = tb["taper_on"]
     etot, n = 0.0, len(pos)
     for i in range(n):
         rho = pair = 0.0
@@ -446,10 +446,12 @@ def _alloy_energy_numpy(pos, types, tb, cutoff):
             if i == j:
                 continue
             r = float(np.sqrt(((pos[i] - pos[j]) ** 2).sum()))
-            if r >= cutoff:
-                continue
             k = types[i] * 2 + types[j]
-            t = min(max((r - ron) / (cutoff - ron), 0.0), 1.0)
+            rc = cutoff if pair_cutoff is None else pair_cutoff[k]
+            ron = ron0 if pair_taper_on is None else pair_taper_on[k]
+            if r >= rc:
+                continue
+            t = min(max((r - ron) / (rc - ron), 0.0), 1.0)
             s = 1.0 - t ** 3 * (10.0 - 15.0 * t + 6.0 * t * t)
             x = r / tb["r0"][k] - 1.0
             rho += tb["xi"][k] ** 2 * np.exp(-2.0 * tb["q"][k] * x) * s
@@ -628,3 +630,38 @@ def test_barostat_one_step_formula_and_relaxation_to_the_pinned_lattice_constant
     for _ in range(8):
         o.step(10, 1.0)
         assert o.list_covers_cutoff()
+
+
+def test_pair_cutoffs_against_numpy_definition_and_defaults():
+    """the paper's RCUT(ity,jty): per-pair cut-offs and switches"""
+    w = workloads.alloy(workloads.config(0, scale=5), 11, pair_cutoffs=True)
+    rng = np.random.default_rng(3)
+    idx = rng.choice(w.n_atoms, 24, replace=False)
+    pos = w.positions[idx] * 0.6 + 20.0
+    types = w.types[idx]
+    kw = dict(pot_kind=0, mass=w.mass, tbsma=w.tbsma, box=np.full(3, 60.0), cutoff=4.9, skin=0.3, velocities=np.zeros((24, 3)),
+              types=types, n_boxes=1)
+    f, e, _ = Oracle(positions=pos, pair_cutoff=w.pair_cutoff, pair_taper_on=w.pair_taper_on, **kw).compute_forces()
+    eref = _alloy_energy_numpy(pos, types, w.tbsma, 4.9, w.pair_cutoff, w.pair_taper_on)
+    assert abs(e.sum() - eref) < 1e-12 * abs(eref)
+    e_glob = Oracle(positions=pos, **kw).compute_forces()[1].sum()
+    assert abs(e_glob - eref) > 1e-6                       # the pair cut-offs do change the energy of this cluster
+    h = 1e-4
+    for a, c in ((1, 0), (9, 2)):
+        def E(dh):
+            p2 = pos.copy(); p2[a, c] += dh
+            return _alloy_energy_numpy(p2, types, w.tbsma, 4.9, w.pair_cutoff, w.pair_taper_on)
+        fd = -((8 * (E(h) - E(-h)) - (E(2 * h) - E(-2 * h))) / (12 * h))
+        assert abs(fd - f[a, c]) < 2e-8 * max(1.0, abs(f[a, c]))
+    # pair cut-offs equal to the global ones == no pair cut-offs, bit for bit; tables: strict per-pair cut
+    for cfg, sc in (("0", 5), ("1", 7)):
+        w0 = workloads.alloy(workloads.config(cfg, scale=sc), 5)
+        same = Oracle(w0, pair_cutoff=np.full(4, w0.cutoff), pair_taper_on=None if cfg == "1" else np.full(4, w0.tbsma["taper_on"]))
+        assert np.array_equal(same.compute_forces()[0], Oracle(w0).compute_forces()[0])
+    wt = workloads.alloy(workloads.config(1, scale=7), 5, pair_cutoffs=True)
+    ft = Oracle(wt).compute_forces()[0]
+    assert np.abs(ft.sum(0)).max() < 1e-11 and not np.allclose(ft, Oracle(workloads.alloy(workloads.config(1, scale=7), 5)).compute_forces()[0])
+    with pytest.raises(OracleError):                       # larger than the list cut-off, or asymmetric
+        Oracle(w0, pair_cutoff=np.full(4, 1.01 * w0.cutoff))
+    with pytest.raises(OracleError):
+        Oracle(w0, pair_cutoff=np.array([5.0, 4.8, 4.9, 5.0]))

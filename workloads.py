@@ -49,6 +49,8 @@ class Workload:
     pot_kind: int = 0               # 0 = TB-SMA analytic, 1 = EAM cubic-Hermite tables
     tbsma: dict | None = None       # A, xi, p, q, r0: (n_types*n_types,) arrays; taper_on: float
     tables: dict | None = None      # nr, dr, f_val, f_der, phi_val, phi_der, nrho, drho, F_val, F_der
+    pair_cutoff: np.ndarray | None = None    # (n_types*n_types,) per-pair cut-offs <= cutoff (paper's RCUT(ity,jty)), or None
+    pair_taper_on: np.ndarray | None = None  # (n_types*n_types,) TB-SMA: start of each pair's switch, or None
     dt: float = 1.0                 # fs
     steps: int = 100
     meta: dict = field(default_factory=dict)
@@ -220,12 +222,13 @@ def config(k: int | str, scale: int | None = None, replica: int = 0) -> Workload
     raise ValueError(f"unknown config {k!r}")
 
 
-def alloy(w: Workload, seed: int, fraction: float = 0.5) -> Workload:
+def alloy(w: Workload, seed: int, fraction: float = 0.5, pair_cutoffs: bool = False) -> Workload:
     """Binary alloy on the sites of `w` (the paper's rho^(ab), V^(ab)):
     a seeded `fraction` of the atoms becomes type 1.  TB-SMA: type 1 gets a second, synthetic parameter set (larger
     atom, different stiffness) and the cross pair (0,1) = (1,0) its own set, so that every entry of the 2x2 parameter
     arrays differs; tables: the three pair tables are the analytic EAM with different (re, beta, A, B) and the two
-    embedding tables differ in F0.  Parameter arrays are indexed [ti * n_types + tj]."""
+    embedding tables differ in F0.  Parameter arrays are indexed [ti * n_types + tj].  `pair_cutoffs`: the three
+    pairs also get their own cut-offs (r_c, 0.93 r_c, 0.97 r_c; TB-SMA: each switch over its last 0.5 A)."""
     rng = np.random.Generator(np.random.PCG64(seed))
     types = (rng.random(w.n_atoms) < fraction).astype(np.int32)
     w2 = Workload(**{**w.__dict__})
@@ -248,6 +251,12 @@ def alloy(w: Workload, seed: int, fraction: float = 0.5) -> Workload:
         w2.tables = dict(nr=t["nr"], dr=t["dr"], nrho=t["nrho"], drho=t["drho"],
                          f_val=pair("f_val"), f_der=pair("f_der"), phi_val=pair("phi_val"), phi_der=pair("phi_der"),
                          F_val=np.concatenate([t["F_val"], t11["F_val"]]), F_der=np.concatenate([t["F_der"], t11["F_der"]]))
+    if pair_cutoffs:
+        rc = w.cutoff
+        w2.pair_cutoff = np.array([rc, 0.93 * rc, 0.93 * rc, 0.97 * rc])
+        if w.pot_kind == 0:
+            w2.pair_taper_on = w2.pair_cutoff - 0.5
+        w2.name += "_rcut"
     return w2
 
 
