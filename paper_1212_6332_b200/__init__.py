@@ -170,6 +170,8 @@ class MDSystem:
             check(lib().md_workspace_bytes(C.byref(d), C.byref(nbytes)))
             self.workspace_bytes = nbytes.value
             self._ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+            if os.environ.get("MD_POISON_WORKSPACE"):            # test hook: the library must never read what it has not written
+                self._ws.fill_(0xAB)
             base = (self._ws.data_ptr() + 255) & ~255
             self._h = C.c_void_p()
             check(lib().md_create(C.byref(d), C.c_void_p(base), nbytes.value, C.byref(self._h)))

@@ -291,6 +291,24 @@ def test_two_systems_interleaved_and_profile_toggle(md):
     assert np.array_equal(a.positions(), ra.positions()) and a.stats()["error_flags"] == 0
 
 
+@pytest.mark.parametrize("case", ["cfg0_perm", "cfg2_small", "cfg4_small", "alloy_tbsma_rcut"])
+def test_garbage_in_the_workspace_is_never_read(md, case, monkeypatch):
+    """the caller's allocation arrives uninitialised: pre-fill it with 0xAB (a list entry of that pattern would index far
+    outside every array) and require the same results as the oracle"""
+    monkeypatch.setenv("MD_POISON_WORKSPACE", "1")
+    w = CASES[case]()
+    o, g = oracle_of(w), md.MDSystem(w)
+    gf, ge, gw = g.compute_forces()
+    of, oe, ow = o.compute_forces()
+    assert np.abs(gf - of).max() <= F_TOL and np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    o.step(40, w.dt)
+    g.step(40, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+    assert np.array_equal(g.neighbors(192)[1][:, :4] >= -1, np.ones((w.n_atoms, 4), bool))
+
+
 def test_run_to_run_determinism(md):
     w = CASES["cfg2_small"]()
     res = []
