@@ -220,31 +220,22 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
   const int zlo = max(cz - 1, 0), zhi = min(cz + 1, ncz - 1);
   int n_all = 0;
-  bool overflow = false;
   // pairs inside r_in (= r_c) now go to the front of the row (k = 0, 1, ...), skin pairs to the back (k = cap-1, cap-2, ...):
   // the two passes run the full pair evaluation only over the front part (md_force.cu)
   int n_in = 0, n_out = 0;
-  auto keep = [&](int j, double r2, unsigned code) {
-    const unsigned entry = (unsigned)j | (code << kIdxBits);
-    if (n_in + n_out < s.cap) {
-      if (r2 < s.rin2) row[nbr_entry(n_in++)] = entry;
-      else row[nbr_entry(s.cap - 1 - n_out++)] = entry;
-    } else {
-      overflow = true;
-    }
-    ++n_all;
-  };
-  // the same without branches (one predicated store), for the PERCELL candidate loop: almost every trip has SOME lane
-  // that accepts its candidate, so a branchy append runs for the whole warp on nearly every candidate
+  // branch-free append (one predicated store): almost every trip has SOME lane that accepts its candidate, so a branchy
+  // append would run for the whole warp on nearly every candidate
+  int n_lost = 0;                                                 // accepted but not stored (row full)
   auto test_keep = [&](int j, double r2, unsigned code) {
     const bool acc = r2 < s.rl2 && j != i;
-    const bool room = n_in + n_out < s.cap;
     const bool in = r2 < s.rin2;
-    const int k = in ? n_in : s.cap - 1 - n_out;
-    if (acc && room) row[nbr_entry(k)] = (unsigned)j | (code << kIdxBits);
-    n_in += (acc && room && in) ? 1 : 0;
-    n_out += (acc && room && !in) ? 1 : 0;
-    n_all += acc ? 1 : 0;
+    const int m_out = s.cap - 1 - n_out;                          // next free entry from the back
+    const bool put = acc && n_in <= m_out;                        // room: n_in + n_out < cap
+    const int k = in ? n_in : m_out;
+    if (put) row[nbr_entry(k)] = (unsigned)j | (code << kIdxBits);
+    n_in += (put && in) ? 1 : 0;
+    n_out += (put && !in) ? 1 : 0;
+    n_lost += (acc && !put) ? 1 : 0;
   };
   for (int ox = -1; ox <= 1; ++ox) {
     int jx = cx + ox;
@@ -312,7 +303,8 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
       }
     }
   }
-  if (overflow || n_all > n_in + n_out) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
+  n_all += n_in + n_out + n_lost;
+  if (n_lost > 0) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
   // the passes read whole groups of four: zero the unused entries of the two partly filled groups
   const int first_out = s.cap - n_out;
   for (int k = n_in; k < min((n_in + 3) & ~3, first_out); ++k) row[nbr_entry(k)] = 0u;
