@@ -259,8 +259,9 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           // in between cannot hold them back), then the four tests
           const unsigned code = kx | (ky << 2) | (kz << 4);
           auto dist2 = [&](const double4 &pj, double &r2) {
-            double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
-            if (code) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
+            // the shift is added unconditionally: d + 0.0 == d, and a test per candidate costs more than three additions
+            const double dx = __dadd_rn(__dsub_rn(pj.x, pi.x), sx), dy = __dadd_rn(__dsub_rn(pj.y, pi.y), sy),
+                         dz = __dadd_rn(__dsub_rn(pj.z, pi.z), sz);
             r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
           };
           int j = jbeg;
