@@ -93,7 +93,7 @@ struct DevSys {
 
 // first entry of the list row of the atom in (tile, lane); entry k is at row[(k >> 2) * 128 + (k & 3)]
 __host__ __device__ inline size_t nbr_row_offset(size_t tile, int cap, int lane) { return (tile * (size_t)(cap >> 2) * 32 + lane) * 4; }
-__host__ __device__ inline size_t nbr_entry(int k) { return (size_t)(k >> 2) * 128 + (k & 3); }
+__host__ __device__ inline unsigned nbr_entry(int k) { return ((unsigned)k >> 2) * 128u + ((unsigned)k & 3u); }   // 32-bit: one IMAD.WIDE per store
 
 // current box edge a: a kernel parameter until a barostat is switched on, device state from then on
 __device__ __forceinline__ double box_edge(const DevSys &s, int a) { return s.dyn_box ? s.st->box[a] : s.L0[a]; }
