@@ -247,6 +247,12 @@ __device__ __forceinline__ double4 gather32(const double4 *p) {
   asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
   return v;
 }
+// base + 32 * idx with one 32 x 32 -> 64 bit multiply-add (the compiler's own sequence is shift, mask, add, add-with-carry)
+__device__ __forceinline__ const double4 *slot_ptr(const double4 *base, unsigned idx) {
+  unsigned long long a;
+  asm("mad.wide.u32 %0, %1, 32, %2;" : "=l"(a) : "r"(idx), "l"((unsigned long long)base));
+  return (const double4 *)a;
+}
 __device__ __forceinline__ int order_token(const PairD &a) { return __double2loint(a.r2); }
 
 // eval2 evaluates two pairs at once: their dependency chains are independent (measured on B200: one dependent DFMA
@@ -258,19 +264,19 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
   const int ng = (n + 3) >> 2, nfull = n >> 2;
   uint4 E = ng > 0 ? ldg_group(row) : none;
   uint4 En = ng > 1 ? ldg_group(row + 32) : none;
-  double4 pA = gather32(pos + MD_GIDX(E.x));                      // slot 0 when there is no such pair: harmless
-  double4 pB = gather32(pos + MD_GIDX(E.y));
+  double4 pA = gather32(slot_ptr(pos, MD_GIDX(E.x)));                      // slot 0 when there is no such pair: harmless
+  double4 pB = gather32(slot_ptr(pos, MD_GIDX(E.y)));
   for (int g = 0; g < nfull; ++g) {
     const PairD a = prep(E.x, pA), b = prep(E.y, pB);
     const int t1 = (order_token(a) | order_token(b)) * zero;
     const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32 + t1) : none;
-    const double4 pC = gather32(pos + (MD_GIDX(E.z) + t1));
-    const double4 pD = gather32(pos + (MD_GIDX(E.w) + t1));
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z) + t1));
+    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.w) + t1));
     eval2(a, b);
     const PairD c = prep(E.z, pC), d = prep(E.w, pD);
     const int t2 = (order_token(c) | order_token(d)) * zero;
-    pA = gather32(pos + (MD_GIDX(En.x) + t2));
-    pB = gather32(pos + (MD_GIDX(En.y) + t2));
+    pA = gather32(slot_ptr(pos, MD_GIDX(En.x) + t2));
+    pB = gather32(slot_ptr(pos, MD_GIDX(En.y) + t2));
     eval2(c, d);
     E = En; En = E2;
   }
@@ -278,7 +284,7 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
   if (rem >= 2) {
     const PairD a = prep(E.x, pA), b = prep(E.y, pB);
     const int t1 = (order_token(a) | order_token(b)) * zero;
-    const double4 pC = gather32(pos + (MD_GIDX(E.z) + t1));
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z) + t1));
     eval2(a, b);
     if (rem == 3) eval1(prep(E.z, pC));
   } else if (rem == 1) {
@@ -296,21 +302,21 @@ __device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n,
   const int ng = (n + 3) >> 2;
   uint4 E = ng > 0 ? ldg_group(last) : none;
   uint4 En = ng > 1 ? ldg_group(last - 32) : none;
-  double4 pA = gather32(pos + MD_GIDX(E.w));
-  double4 pB = gather32(pos + MD_GIDX(E.z));
+  double4 pA = gather32(slot_ptr(pos, MD_GIDX(E.w)));
+  double4 pB = gather32(slot_ptr(pos, MD_GIDX(E.z)));
   for (int g = 0; g < mg; ++g) {
     const int j = g * 4;
     const PairD a = prep(E.w, pA), b = prep(E.z, pB);
     const int t1 = (order_token(a) | order_token(b)) * zero;
     const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32 + t1) : none;
-    const double4 pC = gather32(pos + (MD_GIDX(E.y) + t1));
-    const double4 pD = gather32(pos + (MD_GIDX(E.x) + t1));
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.y) + t1));
+    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.x) + t1));
     body(a, j < n);
     body(b, j + 1 < n);
     const PairD c = prep(E.y, pC), d = prep(E.x, pD);
     const int t2 = (order_token(c) | order_token(d)) * zero;
-    pA = gather32(pos + (MD_GIDX(En.w) + t2));
-    pB = gather32(pos + (MD_GIDX(En.z) + t2));
+    pA = gather32(slot_ptr(pos, MD_GIDX(En.w) + t2));
+    pB = gather32(slot_ptr(pos, MD_GIDX(En.z) + t2));
     body(c, j + 2 < n);
     body(d, j + 3 < n);
     E = En; En = E2;
