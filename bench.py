@@ -60,9 +60,9 @@ SLOTS = {
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two passes, from the committed `ncu --set full`
-# capture of this command on this workload (profiles/r01h_ncu_cfg3a.md); None for workloads without a capture.
-NCU_TRAFFIC = {"3a": {"force": 340.1e6, "density": 312.5e6, "fp64_pipe_active_pct": {"force": 50.3, "density": 41.9},
-                      "source": "profiles/r01h_ncu_cfg3a.md"}}
+# capture of this command on this workload (profiles/r01k_ncu_cfg3a.md); None for workloads without a capture.
+NCU_TRAFFIC = {"3a": {"force": 340.0e6, "density": 312.8e6, "fp64_pipe_active_pct": {"force": 52.9, "density": 42.6},
+                      "source": "profiles/r01k_ncu_cfg3a.md"}}
 
 
 def algorithmic(kind: int, n_atoms: int, list_entries: float, in_cutoff: float) -> dict:
