@@ -232,7 +232,11 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     const int m_out = s.cap - 1 - n_out;                          // next free entry from the back
     const bool put = acc && n_in <= m_out;                        // room: n_in + n_out < cap
     const int k = in ? n_in : m_out;
-    if (put) row[nbr_entry(k)] = (unsigned)j | (code << kIdxBits);
+    if (put) {                                                    // row + 4 * offset with one 32 x 32 -> 64 bit multiply-add
+      unsigned long long a;
+      asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(a) : "r"(nbr_entry(k)), "l"((unsigned long long)row));
+      *(unsigned *)a = (unsigned)j | (code << kIdxBits);
+    }
     n_in += (put && in) ? 1 : 0;
     n_out += (put && !in) ? 1 : 0;
     n_lost += (acc && !put) ? 1 : 0;
