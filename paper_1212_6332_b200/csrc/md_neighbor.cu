@@ -226,10 +226,10 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   // branch-free append (one predicated store): almost every trip has SOME lane that accepts its candidate, so a branchy
   // append would run for the whole warp on nearly every candidate
   int n_lost = 0;                                                 // accepted but not stored (row full)
+  int m_out = s.cap - 1;                                          // next free entry from the back (n_out = cap - 1 - m_out)
   auto test_keep = [&](int j, double r2, unsigned code) {
     const bool acc = r2 < s.rl2 && j != i;
     const bool in = r2 < s.rin2;
-    const int m_out = s.cap - 1 - n_out;                          // next free entry from the back
     const bool put = acc && n_in <= m_out;                        // room: n_in + n_out < cap
     const int k = in ? n_in : m_out;
     if (put) {                                                    // row + 4 * offset with one 32 x 32 -> 64 bit multiply-add
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
       *(unsigned *)a = (unsigned)j | (code << kIdxBits);
     }
     n_in += (put && in) ? 1 : 0;
-    n_out += (put && !in) ? 1 : 0;
+    m_out -= (put && !in) ? 1 : 0;
     n_lost += (acc && !put) ? 1 : 0;
   };
   for (int ox = -1; ox <= 1; ++ox) {
@@ -308,6 +308,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
       }
     }
   }
+  n_out = s.cap - 1 - m_out;
   n_all += n_in + n_out + n_lost;
   if (n_lost > 0) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
   // the passes read whole groups of four: zero the unused entries of the two partly filled groups
