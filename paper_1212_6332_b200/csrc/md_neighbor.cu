@@ -6,6 +6,8 @@
 // device: histogram -> scan -> scatter -> per-cell ordering -> re-order -> list, and every kernel of the
 // chain is launched unconditionally but returns at once unless DevState says a rebuild is due, so that
 // md_step never needs the host to look at the displacement flag.
+#include <type_traits>
+
 #include "md_internal.cuh"
 
 namespace md {
@@ -262,24 +264,27 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           // four candidates per trip: the four loads are issued together (read-only path, so the list stores
           // in between cannot hold them back), then the four tests
           const unsigned code = kx | (ky << 2) | (kz << 4);
-          auto dist2 = [&](const double4 &pj, double &r2) {
-            // the shift is added unconditionally: d + 0.0 == d, and a test per candidate costs more than three additions
-            const double dx = __dadd_rn(__dsub_rn(pj.x, pi.x), sx), dy = __dadd_rn(__dsub_rn(pj.y, pi.y), sy),
-                         dz = __dadd_rn(__dsub_rn(pj.z, pi.z), sz);
-            r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          // runs across the box boundary add the shift (d + (-L) == d - L bit for bit); the others (95 % in a large box) do not
+          auto scan = [&](auto shifted) {
+            auto dist2 = [&](const double4 &pj, double &r2) {
+              double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
+              if (decltype(shifted)::value) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
+              r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            };
+            int j = jbeg;
+            for (; j + 4 <= jend; j += 4) {
+              const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
+              double r0, r1, r2, r3;
+              dist2(p0, r0); dist2(p1, r1); dist2(p2, r2); dist2(p3, r3);
+              test_keep(j, r0, code); test_keep(j + 1, r1, code); test_keep(j + 2, r2, code); test_keep(j + 3, r3, code);
+            }
+            for (; j < jend; ++j) {
+              double r2;
+              dist2(ld_pos(s.pos + j), r2);
+              test_keep(j, r2, code);
+            }
           };
-          int j = jbeg;
-          for (; j + 4 <= jend; j += 4) {
-            const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
-            double r0, r1, r2, r3;
-            dist2(p0, r0); dist2(p1, r1); dist2(p2, r2); dist2(p3, r3);
-            test_keep(j, r0, code); test_keep(j + 1, r1, code); test_keep(j + 2, r2, code); test_keep(j + 3, r3, code);
-          }
-          for (; j < jend; ++j) {
-            double r2;
-            dist2(ld_pos(s.pos + j), r2);
-            test_keep(j, r2, code);
-          }
+          if (code) scan(std::true_type{}); else scan(std::false_type{});
         } else {
           // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
           auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
