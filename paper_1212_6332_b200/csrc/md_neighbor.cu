@@ -234,11 +234,9 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     const bool in = r2 < s.rin2;
     const bool put = acc && n_in <= m_out;                        // room: n_in + n_out < cap
     const int k = in ? n_in : m_out;
-    if (put) {                                                    // row + 4 * offset with one 32 x 32 -> 64 bit multiply-add
-      unsigned long long a;
-      asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(a) : "r"(nbr_entry(k)), "l"((unsigned long long)row));
-      *(unsigned *)a = (unsigned)j | (code << kIdxBits);
-    }
+    // one predicated store, no branch: address = row + 4 * offset by one 32 x 32 -> 64 bit multiply-add
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .u64 a;\n\tsetp.ne.u32 p, %3, 0;\n\tmad.wide.u32 a, %1, 4, %0;\n\t@p st.global.u32 [a], %2;\n\t}"
+                 :: "l"((unsigned long long)row), "r"(nbr_entry(k)), "r"((unsigned)j | (code << kIdxBits)), "r"((unsigned)put) : "memory");
     n_in += (put && in) ? 1 : 0;
     m_out -= (put && !in) ? 1 : 0;
     n_lost += (acc && !put) ? 1 : 0;
