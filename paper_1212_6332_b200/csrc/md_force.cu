@@ -429,17 +429,19 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   // skin part: distance test only; a pair found inside r_c is parked (one slot per lane) and the warp evaluates
   // the parked pairs together when some lane needs its slot again, and once at the end
   const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
-  PairD park = {};
+  // only the ENTRY is parked (one register); the rare evaluation gathers and prepares the pair again
+  unsigned park = 0u;
   bool parked = false;
+  auto flush = [&]() { rho += term1(prep(park, gather32(slot_ptr(s.pos, MD_GIDX(park))))); parked = false; };
   walk_tail(row.last, row.n_out, mg, s.pos, zero, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
-      if (parked) { rho += term1(park); parked = false; }
+      if (parked) flush();
     }
-    if (hit) { park = d; parked = true; }
+    if (hit) { park = d.e; parked = true; }
   });
   if (__any_sync(0xffffffffu, parked)) {
-    if (parked) rho += term1(park);
+    if (parked) flush();
   }
 
   if (!valid) return;
@@ -621,18 +623,18 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
 
   // skin part: distance test only; pairs found inside r_c are parked and evaluated together (see k_density)
   const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
-  PairD park = {};
-  park.r2 = 1.0;
+  unsigned park = 0u;
   bool parked = false;
+  auto flush = [&]() { eval1(prep(park, gather32(slot_ptr(s.posf, MD_GIDX(park)))), acc); parked = false; };
   walk_tail(row.last, row.n_out, mg, s.posf, zero, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
-      if (parked) { eval1(park, acc); parked = false; }
+      if (parked) flush();
     }
-    if (hit) { park = d; parked = true; }
+    if (hit) { park = d.e; parked = true; }
   });
   if (__any_sync(0xffffffffu, parked)) {
-    if (parked) eval1(park, acc);
+    if (parked) flush();
   }
 
   force_finish<OBS>(s, kick, i, valid, ti, acc, sm);
