@@ -387,15 +387,16 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
 template <int KIND, bool MULTI, bool FOLD, bool DYN>
 __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s) {
   __shared__ double tab_sm[kExpTabLen];
-  unsigned tab = 0;
-  LoopConsts lc = {};
-  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
+  // the atom's own loads are issued BEFORE the table staging and its barrier, so that their latency overlaps it
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
   const int i = box * s.npb + (valid ? local : 0);
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.pos[i];
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int ti = MULTI ? (int)pi.w : 0;
   double rho = 0.0, rho2 = 0.0;
 
@@ -580,15 +581,15 @@ template <int KIND, bool MULTI, bool OBS, bool FOLD, bool DYN>
 __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
-  unsigned tab = 0;
-  LoopConsts lc = {};
-  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
   const int i = box * s.npb + (valid ? local : 0);
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.posf[i];
+  unsigned tab = 0;
+  LoopConsts lc = {};
+  if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int ti = MULTI ? s.type[i] : 0;
   ForceAcc<OBS> acc, acc2;
 
