@@ -229,12 +229,10 @@ __device__ __forceinline__ void embed(const DevSys &s, int ti, double rho, doubl
 // cap-1 were in the skin ("tail").
 //
 // Software pipeline.  prep(e, pj) turns a gathered neighbour into a PairD (d = x_j - x_i with its image, r2, w);
-// eval2 / eval1 run the potential on one or two PairDs.  While pairs k, k+1 are evaluated, the gathers of pairs k+2,
-// k+3 and the entries of the group after next are in flight.  ptxas gives every global load of the loop the SAME
-// scoreboard, and a scoreboard wait is a wait for ALL loads outstanding on it: a gather issued before the first use of
-// the previous gather would make that use wait for the new load's full latency (measured: 45 % of the stall samples).
-// So every load address carries `tok * zero`, where tok comes out of the preceding prep and zero is an integer that
-// is 0 at run time but not at compile time: the loads cannot be hoisted above the use of the data they would delay.
+// eval2 / eval1 run the potential on one or two PairDs.  In the source, the gathers of pairs k+2, k+3 and the entries
+// of the group after next are issued before pairs k, k+1 are evaluated; ptxas places them where it likes (it gives
+// every global load of the loop ONE scoreboard and keeps the loads of a trip close to their first use; forcing them
+// earlier through artificial address dependencies was measured and cost 3 %).
 // ------------------------------------------------------------------------------------------------
 struct PairD { double dx, dy, dz, r2, w; unsigned e; };
 
@@ -253,13 +251,12 @@ __device__ __forceinline__ const double4 *slot_ptr(const double4 *base, unsigned
   asm("mad.wide.u32 %0, %1, 32, %2;" : "=l"(a) : "r"(idx), "l"((unsigned long long)base));
   return (const double4 *)a;
 }
-__device__ __forceinline__ int order_token(const PairD &a) { return __double2loint(a.r2); }
 
 // eval2 evaluates two pairs at once: their dependency chains are independent (measured on B200: one dependent DFMA
 // chain per warp tops out at 64 % of the FP64 pipe, two at 77 %, four at 90 %).
 template <class Prep, class Eval2, class Eval1>
-__device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, const double4 *__restrict__ pos, int zero, Prep prep,
-                                          Eval2 eval2, Eval1 eval1) {
+__device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, const double4 *__restrict__ pos, Prep prep, Eval2 eval2,
+                                          Eval1 eval1) {
   const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2, nfull = n >> 2;
   uint4 E = ng > 0 ? ldg_group(row) : none;
@@ -268,23 +265,20 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
   double4 pB = gather32(slot_ptr(pos, MD_GIDX(E.y)));
   for (int g = 0; g < nfull; ++g) {
     const PairD a = prep(E.x, pA), b = prep(E.y, pB);
-    const int t1 = (order_token(a) | order_token(b)) * zero;
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32 + t1) : none;
-    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z) + t1));
-    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.w) + t1));
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : none;
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z)));
+    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.w)));
     eval2(a, b);
     const PairD c = prep(E.z, pC), d = prep(E.w, pD);
-    const int t2 = (order_token(c) | order_token(d)) * zero;
-    pA = gather32(slot_ptr(pos, MD_GIDX(En.x) + t2));
-    pB = gather32(slot_ptr(pos, MD_GIDX(En.y) + t2));
+    pA = gather32(slot_ptr(pos, MD_GIDX(En.x)));
+    pB = gather32(slot_ptr(pos, MD_GIDX(En.y)));
     eval2(c, d);
     E = En; En = E2;
   }
   const int rem = n & 3;                                          // the partly filled last group
   if (rem >= 2) {
     const PairD a = prep(E.x, pA), b = prep(E.y, pB);
-    const int t1 = (order_token(a) | order_token(b)) * zero;
-    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z) + t1));
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z)));
     eval2(a, b);
     if (rem == 3) eval1(prep(E.z, pC));
   } else if (rem == 1) {
@@ -296,8 +290,7 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
 // last = the last group of the row; mg = warp-uniform number of groups (max over the warp of ceil(n/4));
 // body(PairD, active) is called by all 32 lanes.
 template <class Prep, class Body>
-__device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n, int mg, const double4 *__restrict__ pos, int zero, Prep prep,
-                                          Body body) {
+__device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n, int mg, const double4 *__restrict__ pos, Prep prep, Body body) {
   const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2;
   uint4 E = ng > 0 ? ldg_group(last) : none;
@@ -307,16 +300,14 @@ __device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n,
   for (int g = 0; g < mg; ++g) {
     const int j = g * 4;
     const PairD a = prep(E.w, pA), b = prep(E.z, pB);
-    const int t1 = (order_token(a) | order_token(b)) * zero;
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32 + t1) : none;
-    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.y) + t1));
-    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.x) + t1));
+    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32) : none;
+    const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.y)));
+    const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.x)));
     body(a, j < n);
     body(b, j + 1 < n);
     const PairD c = prep(E.y, pC), d = prep(E.x, pD);
-    const int t2 = (order_token(c) | order_token(d)) * zero;
-    pA = gather32(slot_ptr(pos, MD_GIDX(En.w) + t2));
-    pB = gather32(slot_ptr(pos, MD_GIDX(En.z) + t2));
+    pA = gather32(slot_ptr(pos, MD_GIDX(En.w)));
+    pB = gather32(slot_ptr(pos, MD_GIDX(En.z)));
     body(c, j + 2 < n);
     body(d, j + 3 < n);
     E = En; En = E2;
@@ -402,7 +393,6 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
 
   // main part: branch-free.  TB-SMA: the clamped switch makes a pair beyond r_c contribute exactly 0;
   // tables (no switch, reading A9): the strict test r2 < rc2 selects the term.
-  const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
   auto prep = [&](unsigned e, const double4 &pj) {
     PairD d;
     d.r2 = pair_r2<KIND != MD_POT_TBSMA, DYN>(pj, pi, e, s, d.dx, d.dy, d.dz);
@@ -413,7 +403,7 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
     const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)d.w : 0, d.r2);
     return (KIND == MD_POT_TBSMA || d.r2 < (MULTI ? s.rc2p[ti * s.nt + (int)d.w] : s.rc2)) ? term : 0.0;
   };
-  walk_main(row.main, row.n_in, s.pos, zero, prep,
+  walk_main(row.main, row.n_in, s.pos, prep,
             [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
                 const double r2v[2] = {a.r2, b.r2};
@@ -434,7 +424,7 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   unsigned park = 0u;
   bool parked = false;
   auto flush = [&]() { rho += term1(prep(park, gather32(slot_ptr(s.pos, MD_GIDX(park))))); parked = false; };
-  walk_tail(row.last, row.n_out, mg, s.pos, zero, prep, [&](const PairD &d, bool active) {
+  walk_tail(row.last, row.n_out, mg, s.pos, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
       if (parked) flush();
@@ -593,7 +583,6 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   const int ti = MULTI ? s.type[i] : 0;
   ForceAcc<OBS> acc, acc2;
 
-  const int zero = s.N >> 27;                                     // 0 at run time (N <= 2^26): see the walkers
   auto prep = [&](unsigned e, const double4 &pj) {
     PairD d;
     d.r2 = pair_r2<KIND != MD_POT_TBSMA, DYN>(pj, pi, e, s, d.dx, d.dy, d.dz);
@@ -607,7 +596,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     if (KIND != MD_POT_TBSMA && !(d.r2 < (MULTI ? s.rc2p[tp] : s.rc2))) { g = 0.0; V = 0.0; }   // tables: strict cut-off (A9)
     force_accumulate<OBS>(to, g, V, d.dx, d.dy, d.dz);
   };
-  walk_main(row.main, row.n_in, s.posf, zero, prep,
+  walk_main(row.main, row.n_in, s.posf, prep,
             [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
                 const double r2v[2] = {a.r2, b.r2}, fpv[2] = {pi.w + a.w, pi.w + b.w};
@@ -627,7 +616,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   unsigned park = 0u;
   bool parked = false;
   auto flush = [&]() { eval1(prep(park, gather32(slot_ptr(s.posf, MD_GIDX(park)))), acc); parked = false; };
-  walk_tail(row.last, row.n_out, mg, s.posf, zero, prep, [&](const PairD &d, bool active) {
+  walk_tail(row.last, row.n_out, mg, s.posf, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
       if (parked) flush();
