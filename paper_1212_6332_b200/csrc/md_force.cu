@@ -260,12 +260,11 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
   const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2, nfull = n >> 2;
   uint4 E = ng > 0 ? ldg_group(row) : none;
-  uint4 En = ng > 1 ? ldg_group(row + 32) : none;
   double4 pA = gather32(slot_ptr(pos, MD_GIDX(E.x)));                      // slot 0 when there is no such pair: harmless
   double4 pB = gather32(slot_ptr(pos, MD_GIDX(E.y)));
   for (int g = 0; g < nfull; ++g) {
+    const uint4 En = (g + 1 < ng) ? ldg_group(row + (size_t)(g + 1) * 32) : none;   // a whole trip (four pairs) ahead
     const PairD a = prep(E.x, pA), b = prep(E.y, pB);
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(row + (size_t)(g + 2) * 32) : none;
     const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.z)));
     const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.w)));
     eval2(a, b);
@@ -273,7 +272,7 @@ __device__ __forceinline__ void walk_main(const uint4 *__restrict__ row, int n, 
     pA = gather32(slot_ptr(pos, MD_GIDX(En.x)));
     pB = gather32(slot_ptr(pos, MD_GIDX(En.y)));
     eval2(c, d);
-    E = En; En = E2;
+    E = En;
   }
   const int rem = n & 3;                                          // the partly filled last group
   if (rem >= 2) {
