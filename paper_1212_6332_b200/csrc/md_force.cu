@@ -293,13 +293,12 @@ __device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n,
   const uint4 none = make_uint4(0u, 0u, 0u, 0u);
   const int ng = (n + 3) >> 2;
   uint4 E = ng > 0 ? ldg_group(last) : none;
-  uint4 En = ng > 1 ? ldg_group(last - 32) : none;
   double4 pA = gather32(slot_ptr(pos, MD_GIDX(E.w)));
   double4 pB = gather32(slot_ptr(pos, MD_GIDX(E.z)));
   for (int g = 0; g < mg; ++g) {
     const int j = g * 4;
+    const uint4 En = (g + 1 < ng) ? ldg_group(last - (size_t)(g + 1) * 32) : none;
     const PairD a = prep(E.w, pA), b = prep(E.z, pB);
-    const uint4 E2 = (g + 2 < ng) ? ldg_group(last - (size_t)(g + 2) * 32) : none;
     const double4 pC = gather32(slot_ptr(pos, MD_GIDX(E.y)));
     const double4 pD = gather32(slot_ptr(pos, MD_GIDX(E.x)));
     body(a, j < n);
@@ -309,7 +308,7 @@ __device__ __forceinline__ void walk_tail(const uint4 *__restrict__ last, int n,
     pB = gather32(slot_ptr(pos, MD_GIDX(En.z)));
     body(c, j + 2 < n);
     body(d, j + 3 < n);
-    E = En; En = E2;
+    E = En;
   }
 }
 
