@@ -443,6 +443,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     // 2^(j/64), j = 0..63, rounded from long double (64-bit mantissa): the table of exp_scaled() in md_force.cu
     for (int j = 0; j < 64; ++j) s->exp_tab_host[j] = (double)exp2l((long double)j / 64.0L);
     for (int j = 64; j < kExpTabLen; ++j) s->exp_tab_host[j] = 0.0;
+    for (int j = 0; j < 16; ++j) s->exp_tab_host[kExp16Off + j] = (double)exp2l((long double)j / 16.0L);
   }
   if (d->pot_kind == MD_POT_TBSMA) {
     bool fold = true;
@@ -457,6 +458,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
       const long double a_rho = 2.0L * d->q[k] + (fold ? logl((long double)pre_rho) : 0.0L), a_rep = (long double)d->p[k] + (fold ? logl((long double)pre_rep) : 0.0L);
       o.tb.b_rho[k] = 2.0 * d->q[k] / d->r0[k]; o.tb.b_rep[k] = d->p[k] / d->r0[k];
       o.tb.ak_rho[k] = (double)(a_rho * K); o.tb.bk_rho[k] = (double)((long double)o.tb.b_rho[k] * K);
+      o.tb.ak16_rho[k] = (double)(a_rho * K / 4.0L); o.tb.bk16_rho[k] = (double)((long double)o.tb.b_rho[k] * K / 4.0L);
       o.tb.ak_rep[k] = (double)(a_rep * K); o.tb.bk_rep[k] = (double)((long double)o.tb.b_rep[k] * K);
       o.tb.pre_rho[k] = fold ? 1.0 : pre_rho; o.tb.pre_rep[k] = fold ? 1.0 : pre_rep;
       // exp_scaled() has no overflow handling: its argument must stay well inside +-690 for 0 <= r <= r_c + skin
@@ -471,7 +473,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     }
     // loop constants that the passes read from memory into registers (md_force.cu, LoopConsts)
     double *lc = s->exp_tab_host + 64;
-    lc[0] = 1.0 / 120.0; lc[1] = 0.375; lc[2] = 6.0; lc[3] = o.tb.inv_w[0]; lc[4] = o.tb.bk_rho[0]; lc[5] = o.tb.bk_rep[0];
+    lc[0] = 1.0 / 120.0; lc[1] = 0.375; lc[2] = 6.0; lc[3] = o.tb.inv_w[0]; lc[4] = o.tb.bk_rho[0]; lc[5] = o.tb.bk_rep[0]; lc[6] = 1.0 / 5040.0; lc[7] = o.tb.bk16_rho[0];
   } else {
     TableParams &t = o.tab;
     t.nr = d->nr; t.nrho = d->nrho; t.dr = d->dr; t.inv_dr = 1.0 / d->dr; t.drho = d->drho; t.inv_drho = 1.0 / d->drho;

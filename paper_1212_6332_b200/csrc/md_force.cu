@@ -63,9 +63,10 @@ __device__ __forceinline__ double pair_r2(const double4 &pj, const double4 &pi, 
 // registers before the loop (LoopConsts): ptxas cannot rematerialise a global load, so they stay in registers instead
 // of being rebuilt by MOV / LDC pairs for every pair.  The others sit in the constant bank and are used in place.
 __constant__ double kLn2_64 = 0x1.62e42fefa39efp-7;           // ln2/64
-__constant__ double kC3 = 1.0 / 6.0, kC4 = 1.0 / 24.0;
+__constant__ double kC3 = 1.0 / 6.0, kC4 = 1.0 / 24.0, kC5 = 1.0 / 120.0, kC6 = 1.0 / 720.0;
+__constant__ double kLn2_16 = 0x1.62e42fefa39efp-5;           // ln2/16
 
-struct LoopConsts { double c5, c375, six, inv_w, bk_rho, bk_rep; };
+struct LoopConsts { double c5, c375, six, inv_w, bk_rho, bk_rep, c7, bk16_rho; };
 
 __device__ __forceinline__ double lds_opaque(unsigned addr) {
   double v;
@@ -76,6 +77,7 @@ __device__ __forceinline__ LoopConsts load_loop_consts(unsigned tab) {   // tab 
   LoopConsts c;
   c.c5 = lds_opaque(tab + 512); c.c375 = lds_opaque(tab + 520); c.six = lds_opaque(tab + 528);
   c.inv_w = lds_opaque(tab + 536); c.bk_rho = lds_opaque(tab + 544); c.bk_rep = lds_opaque(tab + 552);
+  c.c7 = lds_opaque(tab + 560); c.bk16_rho = lds_opaque(tab + 568);
   return c;
 }
 
@@ -156,6 +158,60 @@ __device__ __forceinline__ void exp_scaled_n(const double (&xk)[NP], unsigned ta
   MD_EACH {
     const double v = fma(T[q], p[q], T[q]);
     out[q] = __hiloint2double(__double2hiint(v) + ((ni[q] >> 6) << 20), __double2loint(v));
+  }
+}
+
+// The density pass is bound by the L1 data pipe, where a 64-entry look-up at random indices costs ~5 wavefronts (bank
+// conflicts).  Its exp therefore uses a 16-entry table 2^(j/16): 16 entries lie in 16 distinct bank pairs, so the
+// look-up is conflict-free (2 wavefronts), and the polynomial goes to degree 7: |r| <= ln2/32, r^8/40320 < 1.3e-18.
+// xk is the exponent in units of ln2/16; tab16 = shared-space address of the 16-entry table; c7 = 1/5040 in a register.
+__device__ __forceinline__ double exp_scaled16(double xk, unsigned tab16, double c7) {
+  constexpr double kMagic = 6755399441055744.0;
+  const double t = xk + kMagic;
+  const double n = t - kMagic;
+  const double r = (xk - n) * kLn2_16;
+  const int ni = __double2loint(t);
+  double T;
+  asm("ld.shared.f64 %0, [%1];" : "=d"(T) : "r"(tab16 + ((unsigned)(ni & 15) << 3)));
+  double p = fma(r, c7, kC6);
+  p = fma(p, r, kC5);
+  p = fma(p, r, kC4);
+  p = fma(p, r, kC3);
+  p = fma(p, r, 0.5);
+  p = fma(p * r, r, r);
+  const double v = fma(T, p, T);
+  return __hiloint2double(__double2hiint(v) + ((ni >> 4) << 20), __double2loint(v));
+}
+
+template <int NP>
+__device__ __forceinline__ void exp_scaled16_n(const double (&xk)[NP], unsigned tab16, double c7, double (&out)[NP]) {
+  constexpr double kMagic = 6755399441055744.0;
+  double t[NP], n[NP], r[NP], T[NP], p[NP];
+  int ni[NP];
+#pragma unroll
+  MD_EACH t[q] = xk[q] + kMagic;
+#pragma unroll
+  MD_EACH { n[q] = t[q] - kMagic; ni[q] = __double2loint(t[q]); }
+#pragma unroll
+  MD_EACH asm("ld.shared.f64 %0, [%1];" : "=d"(T[q]) : "r"(tab16 + ((unsigned)(ni[q] & 15) << 3)));
+#pragma unroll
+  MD_EACH r[q] = (xk[q] - n[q]) * kLn2_16;
+#pragma unroll
+  MD_EACH p[q] = fma(r[q], c7, kC6);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], kC5);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], kC4);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], kC3);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q], r[q], 0.5);
+#pragma unroll
+  MD_EACH p[q] = fma(p[q] * r[q], r[q], r[q]);
+#pragma unroll
+  MD_EACH {
+    const double v = fma(T[q], p[q], T[q]);
+    out[q] = __hiloint2double(__double2hiint(v) + ((ni[q] >> 4) << 20), __double2loint(v));
   }
 }
 
@@ -325,13 +381,13 @@ __device__ __forceinline__ AtomRow atom_row(const DevSys &s, int box, int local,
 }
 
 __device__ __forceinline__ unsigned stage_exp_table(const DevSys &s, double *tab) {
-  if (threadIdx.x < kExpTabLen - 1) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
+  if (threadIdx.x < kExpTabLen && threadIdx.x != kExpAddrSlot) tab[threadIdx.x] = s.exp_tab[threadIdx.x];
   const unsigned a = (unsigned)__cvta_generic_to_shared(tab);
-  if (threadIdx.x == kExpTabLen - 1) reinterpret_cast<unsigned *>(tab + (kExpTabLen - 1))[0] = a;   // the last slot is free
+  if (threadIdx.x == kExpAddrSlot) reinterpret_cast<unsigned *>(tab + kExpAddrSlot)[0] = a;
   __syncthreads();
   // read the address back through an opaque load: ptxas would otherwise recompute it (S2UR + ULEA + MOV) at every use
   unsigned t;
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(t) : "r"(a + 8u * (kExpTabLen - 1)));
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(t) : "r"(a + 8u * kExpAddrSlot));
   return t;
 }
 
@@ -344,7 +400,7 @@ __device__ __forceinline__ double density_term(const DevSys &s, const LoopConsts
     const TbsmaParams &tb = s.tb;
     const double r = r2 * rsqrt_fast(r2, lc.c375);
     const double S = switch_S(switch_t(r, MULTI ? tb.inv_w[tp] : lc.inv_w, tb.t0[tp]), lc.six);
-    double e = exp_scaled(fma(-(MULTI ? tb.bk_rho[tp] : lc.bk_rho), r, tb.ak_rho[tp]), tab, lc.c5);
+    double e = exp_scaled16(fma(-(MULTI ? tb.bk16_rho[tp] : lc.bk16_rho), r, tb.ak16_rho[tp]), tab + 8u * kExp16Off, lc.c7);
     if (!FOLD) e *= tb.pre_rho[tp];
     return e * S;
   } else {
@@ -364,8 +420,8 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
 #pragma unroll
   MD_EACH r[q] = r2[q] * rinv[q];
 #pragma unroll
-  MD_EACH { xh[q] = fma(-lc.bk_rho, r[q], tb.ak_rho[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0[0]); }
-  exp_scaled_n<NP>(xh, tab, lc.c5, eh);
+  MD_EACH { xh[q] = fma(-lc.bk16_rho, r[q], tb.ak16_rho[0]); t[q] = switch_t(r[q], lc.inv_w, tb.t0[0]); }
+  exp_scaled16_n<NP>(xh, tab + 8u * kExp16Off, lc.c7, eh);
 #pragma unroll
   MD_EACH {
     if (!FOLD) eh[q] *= tb.pre_rho[0];

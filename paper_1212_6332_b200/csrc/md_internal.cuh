@@ -14,7 +14,10 @@ constexpr int kIdxBits = 26;                       // neighbour entry = index | 
 constexpr unsigned kIdxMask = (1u << kIdxBits) - 1u;
 constexpr int kMaxAtoms = 1 << kIdxBits;
 constexpr int kPairs = MD_MAX_TYPES * MD_MAX_TYPES;
-constexpr int kExpTabLen = 64 + 8;                  // 2^(j/64) table + the loop constants of the passes (md_force.cu)
+// exp_scaled() of md_force.cu: [0,64) 2^(j/64) (force pass, degree-5 polynomial), [64,80) the loop constants of the
+// passes, [80,96) 2^(j/16) (density pass, degree-7 polynomial: 16 entries sit in 16 distinct bank pairs, so the
+// look-up is free of bank conflicts; the density pass is bound by the L1 data pipe, the force pass is not)
+constexpr int kExpTabLen = 64 + 16 + 16, kExp16Off = 80, kExpAddrSlot = 79;   // [64,80): constants; slot 79: the table's shared address
 constexpr double kAmuToEvFs2PerA2 = 103.642696526805;  // 1 amu (A/fs)^2 in eV
 
 // Device-resident mutable state (one per system).
@@ -37,6 +40,7 @@ struct TbsmaParams {               // per type pair, pre-combined on the host
   // fold != 0: ln(xi^2) and ln(2A) are folded into a_rho / a_rep and pre_* = 1 (all prefactors > 0)
   // ak_* = a_* 64/ln2 and bk_* = b_* 64/ln2: the exponent in units of ln2/64, as exp_scaled() takes it
   double ak_rho[kPairs], bk_rho[kPairs], b_rho[kPairs], pre_rho[kPairs];
+  double ak16_rho[kPairs], bk16_rho[kPairs];   // the same in units of ln2/16 (density pass)
   double ak_rep[kPairs], bk_rep[kPairs], b_rep[kPairs], pre_rep[kPairs];
   // per type pair: switch variable t = clamp(r inv_w + t0, 0, 1), inv_w = 1/(r_c - r_on), t0 = -r_on inv_w;
   // m30_inv_w = -30 inv_w (dS/dr prefactor)
