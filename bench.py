@@ -61,7 +61,7 @@ SLOTS = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two passes, from the committed `ncu --set full`
 # capture of this command on this workload (profiles/r01k_ncu_cfg3a.md); None for workloads without a capture.
-NCU_TRAFFIC = {"3a": {"force": 338.7e6, "density": 314.7e6, "fp64_pipe_active_pct": {"force": 56.4, "density": 43.2},
+NCU_TRAFFIC = {"3a": {"force": 338.6e6, "density": 313.8e6, "fp64_pipe_active_pct": {"force": 56.4, "density": 48.4},
                       "source": "profiles/r01k_ncu_cfg3a.md"}}
 
 
