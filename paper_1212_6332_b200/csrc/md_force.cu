@@ -1,21 +1,23 @@
 // md_force.cu — density pass (paper's G18, Fig.5) and force pass with
-// energy and virial (paper's G22, Fig.6), FP64, one thread per atom.
+// energy and virial (paper's G22, Fig.6), FP64; one thread per atom, or 8 lanes per atom
+// for small systems (k_*_sub).
 //
 // Differences from the paper's kernels:
-//  - atoms are in cell order and the list is a blocked-ELL array, so the list reads are coalesced and the
-//    neighbour gathers hit L1/L2; the list entry and the gathered position of the NEXT pair are in flight while
-//    the current pair is evaluated;
+//  - atoms are in cell order and the list is a blocked-ELL array in 16-byte groups of four entries, so one LDG.128
+//    brings four pairs and the neighbour gathers (one 256-bit load each) hit L1/L2;
 //  - the periodic image of each listed pair is recorded at build time, so there is no min/max logic in
-//    the inner loop and r2 is bit-identical to the canonical expression;
+//    the inner loop;
 //  - pairs that were inside r_c at build time come first in every row: that part of the loop is branch-free
-//    (the switch function is clamped, so a pair that has drifted out contributes exactly 0); the skin pairs
-//    behind them only get the 9-instruction distance test, and the few that have drifted inside r_c are
+//    (the switch function is clamped, so a pair that has drifted out contributes exactly 0) and evaluates two pairs
+//    per step; the skin pairs behind them only get the distance test, and the few that have drifted inside r_c are
 //    parked and evaluated together, so a warp does not run the heavy body for one lane at a time;
 //  - r and 1/r come from one MUFU.RSQ64H seed + one cubic Newton step; exp() has no slow path (its argument
-//    is bounded) and uses a 64-entry 2^(j/64) table in shared memory with a degree-5 polynomial;
+//    is bounded): 2^(j/64) table + degree-5 polynomial in the force pass, conflict-free 2^(j/16) table + degree-7
+//    polynomial in the L1-bound density pass;
 //  - F'(rho_j) travels in the w component of the gathered position (one 32-byte sector per neighbour);
 //  - energy and virial are reduced by warp shuffles into per-block partials and a second deterministic
 //    pass, instead of shared-memory partials summed on the host.
+// What bounds these kernels on B200, and what was tried: DESIGN.md section 6.
 #include "md_internal.cuh"
 
 namespace md {
