@@ -105,9 +105,13 @@ typedef struct {
   int neighbor_capacity;          /* list capacity per atom in use */
   long kernel_launches;           /* CUDA kernels this system has enqueued since md_create (host-side count) */
   long list_entries;              /* sum over atoms of the list lengths of the last build (directed pairs) */
+  int graph_active;               /* 1: the last md_step replayed the CUDA graph of one step (MD_OPT_GRAPH); 0: plain launches */
+  int graph_error;                /* cudaError_t of a failed graph build (0: none).  md_step then runs the same kernels as
+                                     plain launches for the life of the system (or until MD_OPT_GRAPH is set to 1 again) */
 } md_stats;
 
-/* Bytes of device workspace md_create needs for this description (pointers in *d are not read). */
+/* Bytes of device workspace md_create needs for this description.  No pointer in *d is read (they may be NULL or
+ * not yet valid); the per-pair arrays pair_cutoff / pair_taper_on are validated by md_create. */
 int md_workspace_bytes(const md_desc *d, size_t *bytes);
 
 /* Build a system: copies positions/velocities/types/potential into the workspace (device pointer,
@@ -191,7 +195,9 @@ int md_profile_reset(md_system *s);
 const char *md_kernel_name(int kernel_class);
 
 /* Diagnostic: measured FP64 issue rate of this device, in DFMA thread-instructions per second, from a
- * register-resident kernel of independent DFMA chains on every SM (the ALU roofline denominator). */
+ * register-resident kernel of independent DFMA chains on every SM (the ALU roofline denominator).  Not part of the
+ * MD path: it needs no md_system and is the one entry point that allocates (16 bytes, cudaMalloc / cudaFree inside
+ * the call) and synchronises the device. */
 int md_fp64_dfma_rate(void *stream, double *dfma_per_s, double *sm_clock_mhz);
 
 const char *md_strerror(int status);

@@ -29,6 +29,7 @@ struct oracle_system {
   double thermo_Te, thermo_tau;          /* electron-bath thermostat, eq.(4); tau <= 0: off */
   double baro_P0, baro_tau;              /* Berendsen barostat, eq.(5); tau <= 0: off */
   int obs_stale;                         /* the barostat scaled x after the last force evaluation */
+  int f_prescale;                        /* f holds the forces of the coordinates before that scaling: queries keep them */
   double *x, *v, *f, *xref, *m;          /* m: per type, eV fs^2/A^2 */
   int *type;
   int kind;
@@ -360,12 +361,23 @@ static int forces_internal(oracle_system *s) {
   return ORACLE_OK;
 }
 
+/* Force evaluation on behalf of a QUERY (forces, energies, pressure asked for between steps).  After a barostat step
+ * (reading B1) the observables belong to the scaled coordinates, while the next first half-kick uses the forces
+ * of the unscaled ones: a query must not change the trajectory, so s->f is put back after the evaluation. */
+static int forces_for_query(oracle_system *s, double *forces_out) {
+  const size_t n3 = 3 * (size_t)s->N;
+  double *keep = (s->forces_valid && s->f_prescale) ? dup_d(s->f, n3) : NULL;
+  int rc = forces_internal(s);
+  if (rc == ORACLE_OK && forces_out) memcpy(forces_out, s->f, n3 * sizeof(double));
+  if (keep) { if (rc == ORACLE_OK) memcpy(s->f, keep, n3 * sizeof(double)); free(keep); }
+  return rc;
+}
+
 int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, double *virial) {
   int rc;
   if (!s) return ORACLE_EINVAL;
   if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
-  if ((rc = forces_internal(s)) != ORACLE_OK) return rc;
-  if (forces) memcpy(forces, s->f, 3 * (size_t)s->N * sizeof(double));
+  if ((rc = forces_for_query(s, forces)) != ORACLE_OK) return rc;
   if (e_atom) memcpy(e_atom, s->eatom, (size_t)s->N * sizeof(double));
   if (virial) memcpy(virial, s->virial, 6 * (size_t)s->nb * sizeof(double));
   return ORACLE_OK;
@@ -406,7 +418,7 @@ static double pressure_now(const oracle_system *s) {
 int oracle_get_pressure(oracle_system *s, double *P) {
   int rc;
   if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
-  if ((!s->forces_valid || s->obs_stale) && (rc = forces_internal(s)) != ORACLE_OK) return rc;
+  if ((!s->forces_valid || s->obs_stale) && (rc = forces_for_query(s, NULL)) != ORACLE_OK) return rc;
   *P = pressure_now(s);
   return ORACLE_OK;
 }
@@ -449,12 +461,14 @@ int oracle_step(oracle_system *s, int n, double dt) {
     s->st.last_max_disp2 = maxd2;
     if (maxd2 > thr && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
     if ((rc = forces_internal(s)) != ORACLE_OK) return rc;
+    s->f_prescale = 0;
     for (int i = 0; i < N; ++i) half_kick(s, i, dt);
     if (s->baro_tau > 0.0) {
       const double mu = cbrt(1.0 - (dt / s->baro_tau) * (s->baro_P0 - pressure_now(s)));
       for (int i = 0; i < 3 * N; ++i) s->x[i] *= mu;
       for (int a = 0; a < 3; ++a) s->L[a] *= mu;
       s->obs_stale = 1;     /* energies / pressure on request are re-evaluated; the next half-kick keeps these forces */
+      s->f_prescale = 1;
     }
     s->st.steps += 1;
   }
@@ -464,7 +478,7 @@ int oracle_step(oracle_system *s, int n, double dt) {
 int oracle_get_positions(oracle_system *s, double *x) { memcpy(x, s->x, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
 int oracle_get_velocities(oracle_system *s, double *v) { memcpy(v, s->v, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
 int oracle_set_positions(oracle_system *s, const double *x) {
-  memcpy(s->x, x, 3 * (size_t)s->N * sizeof(double)); s->have_list = 0; s->forces_valid = 0; return ORACLE_OK;
+  memcpy(s->x, x, 3 * (size_t)s->N * sizeof(double)); s->have_list = 0; s->forces_valid = 0; s->f_prescale = 0; return ORACLE_OK;
 }
 int oracle_set_velocities(oracle_system *s, const double *v) { memcpy(s->v, v, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
 
@@ -488,7 +502,7 @@ int oracle_get_densities(oracle_system *s, double *rho, double *fp) {
 int oracle_get_energies(oracle_system *s, double *epot, double *ekin) {
   int rc;
   if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
-  if ((!s->forces_valid || s->obs_stale) && (rc = forces_internal(s)) != ORACLE_OK) return rc;
+  if ((!s->forces_valid || s->obs_stale) && (rc = forces_for_query(s, NULL)) != ORACLE_OK) return rc;
   for (int b = 0; b < s->nb; ++b) {
     long double ep = 0, ek = 0;
     for (int i = b * s->npb; i < (b + 1) * s->npb; ++i) {

@@ -40,7 +40,8 @@ class MdDesc(C.Structure):
 
 class MdStats(C.Structure):
     _fields_ = [("steps", C.c_long), ("rebuilds", C.c_long), ("max_neighbors", C.c_int), ("error_flags", C.c_int),
-                ("last_max_disp2", C.c_double), ("neighbor_capacity", C.c_int), ("kernel_launches", C.c_long), ("list_entries", C.c_long)]
+                ("last_max_disp2", C.c_double), ("neighbor_capacity", C.c_int), ("kernel_launches", C.c_long), ("list_entries", C.c_long),
+                ("graph_active", C.c_int), ("graph_error", C.c_int)]
 
 
 class MDError(RuntimeError):

@@ -48,7 +48,8 @@ struct Bump {
 
 struct Geometry { int nc[3], tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
 
-static int geometry(const md_desc *d, Geometry &g) {
+// check_pairs: also validate the optional per-pair host arrays (md_create); the size query reads no pointer of *d
+static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
   if (!d || d->n_atoms <= 0 || d->n_boxes <= 0 || d->n_types <= 0 || d->n_types > MD_MAX_TYPES) return MD_EINVAL;
   if (d->n_atoms % d->n_boxes || d->n_atoms > kMaxAtoms) return MD_EINVAL;
   if (!(d->cutoff > 0.0) || !(d->skin >= 0.0) || !isfinite(d->cutoff) || !isfinite(d->skin)) return MD_EINVAL;
@@ -57,7 +58,7 @@ static int geometry(const md_desc *d, Geometry &g) {
   if (d->pot_kind == MD_POT_EAM_TABLE && (double)(d->nr - 1) * d->dr < d->cutoff * (1.0 - 1e-12)) return MD_EINVAL;
   if (d->pot_kind == MD_POT_TBSMA && !(d->taper_on < d->cutoff)) return MD_EINVAL;
   if (d->max_neighbors < 0) return MD_EINVAL;
-  for (int a = 0; a < d->n_types; ++a)
+  for (int a = 0; check_pairs && a < d->n_types; ++a)
     for (int b = 0; b < d->n_types; ++b) {
       const int k = a * d->n_types + b, kt = b * d->n_types + a;
       const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff;
@@ -280,6 +281,22 @@ static int forces_sequence(md_system *s, bool observables, double half_dt) {
   return MD_OK;
 }
 
+// Force evaluation on behalf of a QUERY (md_compute_forces, md_get_energies, md_get_pressure between steps).  After a
+// barostat step the observables belong to the SCALED coordinates, while the next first half-kick must use the forces of
+// the unscaled ones whether or not anybody asked in between (reading B1): frc is stashed in vel_tmp (free
+// outside the rebuild chain; a query cannot trigger a rebuild, the step's own decision consumed the displacement) and
+// put back by query_restore() once the caller has read what it wanted from frc.
+static int query_forces(md_system *s, bool *stashed) {
+  const size_t bytes = 3 * (size_t)s->d.N * sizeof(double);
+  *stashed = s->frc_keep && s->forces_valid;
+  if (*stashed && cudaMemcpyAsync(s->d.vel_tmp, s->d.frc, bytes, cudaMemcpyDeviceToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
+  return forces_sequence(s, true, 0.0);
+}
+static int query_restore(md_system *s, bool stashed) {
+  if (!stashed) return MD_OK;
+  return check_cuda(cudaMemcpyAsync(s->d.frc, s->d.vel_tmp, 3 * (size_t)s->d.N * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+}
+
 static void drop_step_graph(md_system *s) {
   if (s->step_exec) cudaGraphExecDestroy(s->step_exec);
   if (s->step_graph) cudaGraphDestroy(s->step_graph);
@@ -297,7 +314,11 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
   // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot capture);
   // nothing executes during capture, and the graph is launched on the caller's stream
   cudaStream_t user = s->stream, st = nullptr;
-  if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); s->opt_graph = false; return MD_ECUDA; }
+  if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) {
+    const cudaError_t err = cudaGetLastError();
+    s->graph_error = err != cudaSuccess ? (int)err : (int)cudaErrorUnknown; s->opt_graph = false;
+    return MD_ECUDA;
+  }
   s->stream = st;
   cudaGraph_t g = nullptr;
   cudaGraphConditionalHandle cond;
@@ -314,7 +335,11 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
     ok = launch_kick_drift(s, dt) == 0 && launch_decide(s, cond, true) == 0;
     head = s->launches - l0;
     cudaStreamCaptureStatus cs;
+#if CUDART_VERSION >= 13000
+    if (ok) ok = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, nullptr, &ndeps) == cudaSuccess && ndeps == 1;   // + edge data
+#else
     if (ok) ok = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, &ndeps) == cudaSuccess && ndeps == 1;
+#endif
     if (ok) last = deps[0];
     ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
   }
@@ -324,7 +349,11 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
     cp.conditional.handle = cond;
     cp.conditional.type = cudaGraphCondTypeIf;
     cp.conditional.size = 1;
+#if CUDART_VERSION >= 13000
+    ok = cudaGraphAddNode(&cnode, g, &last, nullptr, 1, &cp) == cudaSuccess;     // + dependency edge data
+#else
     ok = cudaGraphAddNode(&cnode, g, &last, 1, &cp) == cudaSuccess;
+#endif
     if (ok) {
       cudaGraph_t bodyg = cp.conditional.phGraph_out[0];
       ok = cudaStreamBeginCaptureToGraph(st, bodyg, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
@@ -350,7 +379,10 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
   s->stream = user;
   cudaStreamDestroy(st);
   if (!ok) {
-    const cudaError_t err = cudaGetLastError();      // fall back to plain launches (e.g. a driver without conditional nodes)
+    // fall back to plain launches (e.g. a driver without conditional nodes): same kernels, same results; the fallback is
+    // visible to the caller as md_stats.graph_error != 0 and md_stats.graph_active == 0
+    const cudaError_t err = cudaGetLastError();
+    s->graph_error = err != cudaSuccess ? (int)err : (int)cudaErrorUnknown;
     if (getenv("MD_DEBUG")) fprintf(stderr, "md: step graph unavailable (%s; head %ld body %ld tail %ld, deps %zu)\n", cudaGetErrorString(err), head, body, tail, ndeps);
     if (g) cudaGraphDestroy(g);
     s->opt_graph = false;
@@ -395,7 +427,7 @@ const char *md_kernel_name(int c) {
 
 int md_workspace_bytes(const md_desc *d, size_t *bytes) {
   Geometry g;
-  int rc = geometry(d, g);
+  int rc = geometry(d, g, false);
   if (rc != MD_OK) return rc;
   if (!bytes) return MD_EINVAL;
   *bytes = layout(d, g, nullptr, nullptr);
@@ -404,7 +436,7 @@ int md_workspace_bytes(const md_desc *d, size_t *bytes) {
 
 int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) {
   Geometry g;
-  int rc = geometry(d, g);
+  int rc = geometry(d, g, true);
   if (rc != MD_OK) return rc;
   if (!out || !workspace || !d->positions || !d->types || !d->mass) return MD_EINVAL;
   if (((uintptr_t)workspace & 255) || bytes < layout(d, g, nullptr, nullptr)) return MD_EINVAL;
@@ -423,6 +455,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
   s->thermo_Te = 0.0; s->thermo_tau = 0.0; s->baro_P0 = 0.0; s->baro_tau = 0.0;
   s->step_graph = nullptr; s->step_exec = nullptr; s->step_dt = 0.0; s->step_obs = false; s->step_kernels = s->body_kernels = 0;
+  s->graph_error = 0; s->last_step_graph = false; s->frc_keep = false;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
   o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
@@ -530,7 +563,7 @@ int md_set_option(md_system *s, int option, int value) {
   switch (option) {
     case MD_OPT_STEP_OBSERVABLES: s->opt_step_obs = value != 0; return MD_OK;
     case MD_OPT_PROFILE: s->opt_profile = value != 0; return MD_OK;
-    case MD_OPT_GRAPH: s->opt_graph = value != 0; return MD_OK;
+    case MD_OPT_GRAPH: s->opt_graph = value != 0; if (value) s->graph_error = 0; return MD_OK;   // switching it on retries a failed build
     case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
   }
   return MD_EINVAL;
@@ -566,7 +599,8 @@ int md_get_pressure(md_system *s, double *P) {
   if (!s || !P) return MD_EINVAL;
   int rc;
   if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
-  if (!(s->forces_valid && s->observables_valid) && (rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+  bool stashed = false;
+  if (!(s->forces_valid && s->observables_valid) && ((rc = query_forces(s, &stashed)) != MD_OK || (rc = query_restore(s, stashed)) != MD_OK)) return rc;
   if (launch_pressure(s) != 0) return MD_ECUDA;
   if (cudaMemcpyAsync(P, &s->d.st->pressure, sizeof(double), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
   return sync_and_flags(s);
@@ -577,7 +611,7 @@ int md_build_neighbors(md_system *s) {
   int rc = request_rebuild(s);
   if (rc != MD_OK) return rc;
   if (launch_rebuild_chain(s) != 0) return MD_ECUDA;
-  s->have_list = true; s->forces_valid = false; s->observables_valid = false;
+  s->have_list = true; s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;
   return MD_OK;
 }
 
@@ -585,7 +619,8 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
   if (!s) return MD_EINVAL;
   int rc;
   if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
-  if ((rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+  bool stashed = false;
+  if ((rc = query_forces(s, &stashed)) != MD_OK) return rc;
   const DevSys &o = s->d;
   bool any_host = false, h;
   double *scratch = (double *)s->stage;
@@ -597,6 +632,7 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
       any_host = true;
     }
   }
+  if ((rc = query_restore(s, stashed)) != MD_OK) return rc;
   if (e_atom) {
     if (on_device(e_atom)) ++s->launches, k_get_scalar<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.eatom, e_atom);
     else {
@@ -627,7 +663,9 @@ int md_step(md_system *s, int n, double dt) {
       if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) return MD_ECUDA;
     s->launches += (long)n * s->step_kernels;
     s->have_list = true; s->forces_valid = true; s->observables_valid = obs && !baro;
+    s->last_step_graph = true;
   } else {
+    s->last_step_graph = false;
     for (int k = 0; k < n; ++k) {
       if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
       if ((rc = forces_sequence(s, obs, 0.5 * dt)) != MD_OK) return rc;
@@ -635,6 +673,7 @@ int md_step(md_system *s, int n, double dt) {
     }
     if (baro) s->observables_valid = false;          // energies and virial on request belong to the scaled positions
   }
+  s->frc_keep = baro;
   s->steps += n;
   return MD_OK;
 }
@@ -666,7 +705,7 @@ int md_set_positions(md_system *s, const double *x) {
     src = (const double *)s->stage;
   }
   ++s->launches, k_set_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, src, s->have_list ? 1 : 0);
-  s->forces_valid = false; s->observables_valid = false;
+  s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;
   if (src != x && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;   // the host buffer may be reused
   return check_cuda(cudaGetLastError());
 }
@@ -750,7 +789,8 @@ int md_get_energies(md_system *s, double *epot, double *ekin) {
   const DevSys &o = s->d;
   if (epot) {
     if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
-    if (!(s->forces_valid && s->observables_valid) && (rc = forces_sequence(s, true, 0.0)) != MD_OK) return rc;
+    bool stashed = false;
+    if (!(s->forces_valid && s->observables_valid) && ((rc = query_forces(s, &stashed)) != MD_OK || (rc = query_restore(s, stashed)) != MD_OK)) return rc;
     if ((rc = deliver(s, epot, o.box_epot, (size_t)o.nb * sizeof(double), nullptr)) != MD_OK) return rc;
   }
   if (ekin) {
@@ -767,6 +807,7 @@ int md_get_stats(md_system *s, md_stats *out) {
   if (cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   out->steps = s->steps; out->rebuilds = (long)st.rebuilds; out->max_neighbors = st.max_neighbors;
   out->error_flags = st.error_flags; out->last_max_disp2 = st.last_maxd2; out->neighbor_capacity = s->d.cap; out->kernel_launches = s->launches + (long)st.graph_body_runs * s->body_kernels; out->list_entries = (long)st.list_entries;
+  out->graph_active = s->last_step_graph ? 1 : 0; out->graph_error = s->graph_error;
   return MD_OK;
 }
 

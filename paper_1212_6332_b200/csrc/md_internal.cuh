@@ -117,6 +117,9 @@ struct md_system {
   bool opt_step_obs, opt_profile, opt_graph;
   // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
   cudaGraph_t step_graph; cudaGraphExec_t step_exec; double step_dt; bool step_obs; int step_kernels, body_kernels;
+  int graph_error;                 // cudaError_t of a failed step-graph build (0: none); md_step then uses plain launches
+  bool last_step_graph;            // the last md_step replayed the graph
+  bool frc_keep;                   // frc holds the forces of the coordinates BEFORE the barostat scaled them: queries must not replace them
   int opt_force_variant;
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];

@@ -97,6 +97,18 @@ def main():
         put(f"{tag}.n_in_cutoff", sum(c for m, c in shells("bcc", a, rc)))
         put(f"{tag}.n_in_list", sum(c for m, c in shells("bcc", a, rc + mpf("0.3"))))
 
+    # F(rho) above the last node of its table (reading A8: linear continuation F(rho_max) + F'(rho_max)(rho - rho_max)):
+    # the Fe-form EAM with rho_max = 8 < rho_lattice = 10.76, so every atom of the perfect crystal sits on the continuation
+    a, rc, re, rmax = mpf("2.855"), mpf("5.0"), mpf("2.4725"), mpf(8)
+    _, pair, rho = eam(a, rc, re, a)
+    Fmax, Fpmax = -mpf("2.5") * sqrt(rmax / 20), -mpf("2.5") / (2 * sqrt(20 * rmax))
+    put("fe_rhomax8.E", Fmax + Fpmax * (rho - rmax) + pair); put("fe_rhomax8.Fp", Fpmax)
+
+    def e_cont(x):
+        _, pr, rh = eam(x, rc, re, a)
+        return Fmax + Fpmax * (rh - rmax) + pr
+    put("fe_rhomax8.W", -a * diff(e_cont, a))
+
     # Cu dimer, eq.(1) for two atoms: E = 2 [ F(f(r)) + V(r)/2 ], force on atom 1 along (r1-r2)/r is -dE/dr
     def dimer(r, ron=mpf("4.4"), rc=mpf("4.9")):
         s, x = switch(r, ron, rc), r / CU["r0"] - 1

@@ -41,7 +41,33 @@ CASES = {
     # per-pair cut-offs, the paper's RCUT(ity,jty): r_c, 0.93 r_c, 0.97 r_c
     "alloy_tbsma_rcut": lambda: workloads.alloy(workloads.config("3a", scale=10), 24, pair_cutoffs=True),
     "alloy_tables_rcut": lambda: workloads.alloy(workloads.config(1, scale=10), 25, pair_cutoffs=True),
+    # three and four species (MD_MAX_TYPES = 4): every one of the n(n+1)/2 parameter sets / tables / cut-offs differs
+    "alloy3_tbsma_rcut": lambda: workloads.alloy(workloads.config("3a", scale=10), 26, n_types=3, pair_cutoffs=True),
+    "alloy4_tbsma": lambda: workloads.alloy(workloads.config("3a", scale=10), 27, n_types=4),
+    "alloy4_tbsma_boxes_rcut": lambda: workloads.alloy(workloads.config(2, scale=5), 28, n_types=4, pair_cutoffs=True),
+    "alloy3_tables": lambda: workloads.alloy(workloads.config(1, scale=10), 29, n_types=3),
+    "alloy4_tables_rcut": lambda: workloads.alloy(workloads.config(1, scale=10), 30, n_types=4, pair_cutoffs=True),
+    # prefactors that cannot be folded into the exponent (xi = 0 for one pair / for all: the kernels' FOLD = false variants)
+    "tbsma_xi0_cross": lambda: _xi0(workloads.alloy(workloads.config("3a", scale=10), 31), cross_only=True),
+    "born_mayer": lambda: _xi0(workloads.config("3a", scale=10), cross_only=False),
+    "born_mayer_boxes": lambda: _xi0(workloads.config(2, scale=6), cross_only=False),
+    # F(rho) above the last node of its table (reading A8): every atom / about half of the atoms on the linear continuation
+    "cfg1_rhomax8": lambda: workloads.bcc_eam(10, 2.855, 2.4725, 5.0, "Fe", seed=41, rho_max=8.0),
+    "cfg1_rhomax_mid": lambda: workloads.bcc_eam(10, 2.855, 2.4725, 5.0, "Fe", seed=42, rho_max=10.76),
 }
+NEW_VARIANT_CASES = ["alloy3_tbsma_rcut", "alloy4_tbsma", "alloy4_tbsma_boxes_rcut", "alloy3_tables", "alloy4_tables_rcut",
+                     "tbsma_xi0_cross", "born_mayer", "born_mayer_boxes", "cfg1_rhomax8", "cfg1_rhomax_mid"]
+
+
+def _xi0(w, cross_only):
+    """xi = 0: no many-body term for that pair (all pairs: a Born-Mayer pair potential, PAPER.md:75 with F = 0)."""
+    w.tbsma = {k: (np.array(v, dtype=np.float64, copy=True) if k != "taper_on" else v) for k, v in w.tbsma.items()}
+    if cross_only:
+        w.tbsma["xi"][[1, 2]] = 0.0
+    else:
+        w.tbsma["xi"][:] = 0.0
+    w.name += "_xi0"
+    return w
 
 
 def _noncubic():
@@ -85,6 +111,9 @@ def test_density_force_energy_virial(md, case):
     assert np.abs(gfp - ofp).max() <= 1e-12 * np.abs(ofp).max()
     assert np.abs(gf - of).max() <= F_TOL
     assert np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    if case.startswith("cfg1_rhomax"):                       # the case does reach the continuation branch
+        rmax = w.tables["drho"] * (w.tables["nrho"] - 1)
+        assert (orho >= rmax).sum() > 100 and ((orho < rmax).sum() > 100 or case == "cfg1_rhomax8")
     oep, oek = o.energies()
     gep, gek = g.energies()
     assert np.abs(gep - oep).max() <= E_REL * np.abs(oep).max()
@@ -98,7 +127,7 @@ def test_density_force_energy_virial(md, case):
 @pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 100), ("cfg1_small", 100), ("cfg2_small", 100),
                                          ("cfg3b_small", 40), ("cfg4_small", 100), ("alloy_tbsma", 100),
                                          ("alloy_tbsma_boxes", 60), ("alloy_tables", 100), ("alloy_tbsma_rcut", 100),
-                                         ("alloy_tables_rcut", 100)])
+                                         ("alloy_tables_rcut", 100)] + [(c, 60) for c in NEW_VARIANT_CASES])
 def test_trajectory(md, case, nsteps):
     w = CASES[case]()
     o = oracle_of(w)
@@ -138,7 +167,7 @@ def test_step_with_observables_matches_plain_step(md):
 
 @pytest.mark.parametrize("variant", [1, 2])
 @pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small", "alloy_tbsma",
-                                  "alloy_tables", "alloy_tbsma_rcut", "alloy_tables_rcut"])
+                                  "alloy_tables", "alloy_tbsma_rcut", "alloy_tables_rcut"] + NEW_VARIANT_CASES)
 def test_both_pass_variants(md, case, variant):
     """One thread per atom (what large systems run) and 8 lanes per atom (small systems), forced on the same input."""
     w = CASES[case]()
@@ -247,6 +276,26 @@ def test_barostat_trajectory(md, case, graph):
     o2 = oracle_of(w2, positions=g.positions())
     o2.build_neighbors()
     assert np.array_equal(g.neighbors(192)[1], o2.neighbors(192)[1])
+
+
+@pytest.mark.parametrize("graph", [0, 1])
+def test_barostat_queries_do_not_change_the_trajectory(md, graph):
+    """reading B1: after a scaled step the next first half-kick keeps the forces of the unscaled coordinates; asking for
+    forces / energies / pressure in between re-evaluates them at the scaled coordinates without touching that."""
+    w = CASES["cfg0"]()
+    a, b, o = md.MDSystem(w), md.MDSystem(w), oracle_of(w)
+    for x in (a, b, o):
+        x.set_barostat(0.0, 20.0)
+    a.set_option(md.MD_OPT_GRAPH, graph); b.set_option(md.MD_OPT_GRAPH, graph)
+    for _ in range(6):
+        a.step(5, 1.0); b.step(5, 1.0); o.step(5, 1.0)
+        fq = b.compute_forces()[0]; b.energies(); b.pressure()
+        assert np.array_equal(fq, b.compute_forces(device_out=True)[0].cpu().numpy())
+        assert np.abs(fq - o.compute_forces()[0]).max() <= F_TOL
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    d = b.positions() - o.positions()
+    d -= np.round(d / o.box()) * o.box()
+    assert np.abs(d).max() <= X_TOL and b.stats()["graph_active"] == graph and b.stats()["graph_error"] == 0
 
 
 def test_barostat_relaxes_perfect_lattice_to_closed_form_and_guards(md):

@@ -436,8 +436,8 @@ def test_isolated_atom_and_empty_neighbourhood():
 
 
 # ---------------------------------------------------------------- binary alloys (PAPER.md:78 rho^(ab), V^(ab))
-def _alloy_energy_numpy(pos, types, tb, cutoff, pair_cutoff=None, pair_taper_on=None):
-    """eq.(1) with type-pair parameters written out in numpy (direct double loop, float64); index [ti*2 + tj]."""
+def _alloy_energy_numpy(pos, types, tb, cutoff, pair_cutoff=None, pair_taper_on=None, nt=2):
+    """eq.(1) with type-pair parameters written out in numpy (direct double loop, float64); index [ti*nt + tj]."""
     ron0 = tb["taper_on"]
     etot, n = 0.0, len(pos)
     for i in range(n):
@@ -446,7 +446,7 @@ def _alloy_energy_numpy(pos, types, tb, cutoff, pair_cutoff=None, pair_taper_on=
             if i == j:
                 continue
             r = float(np.sqrt(((pos[i] - pos[j]) ** 2).sum()))
-            k = types[i] * 2 + types[j]
+            k = types[i] * nt + types[j]
             rc = cutoff if pair_cutoff is None else pair_cutoff[k]
             ron = ron0 if pair_taper_on is None else pair_taper_on[k]
             if r >= rc:
@@ -624,6 +624,17 @@ def test_barostat_one_step_formula_and_relaxation_to_the_pinned_lattice_constant
     assert np.array_equal(a.positions(), b.positions()) and np.array_equal(b.box(), workloads.config(0).box)
     with pytest.raises(OracleError):
         Oracle(workloads.config(2, scale=2)).set_barostat(0.0, 5.0)
+    # a read-only query between steps does not change the trajectory (reading B1: the next first half-kick keeps the
+    # forces of the unscaled coordinates whether or not energies / pressure / forces were asked for in between)
+    a, b = Oracle(workloads.config(0)), Oracle(workloads.config(0))
+    for o in (a, b):
+        o.set_barostat(0.0, 20.0)
+    for _ in range(6):
+        a.step(5, 1.0); b.step(5, 1.0)
+        fq = b.compute_forces()[0]; b.energies(); b.pressure(); fq2 = b.compute_forces()[0]
+        assert np.array_equal(fq, fq2)
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    assert np.abs(fq - Oracle(workloads.config(0), positions=b.positions(), box=b.box()).compute_forces()[0]).max() < 1e-12
     # thermal run under pressure control keeps the list valid (x_ref is not scaled: the rebuild rule sees the scaling)
     o = Oracle(workloads.config(0))
     o.set_barostat(0.0, 20.0)
@@ -665,3 +676,107 @@ def test_pair_cutoffs_against_numpy_definition_and_defaults():
         Oracle(w0, pair_cutoff=np.full(4, 1.01 * w0.cutoff))
     with pytest.raises(OracleError):
         Oracle(w0, pair_cutoff=np.array([5.0, 4.8, 4.9, 5.0]))
+
+
+# ---------------------------------------------------------------- three and four species (MD_MAX_TYPES = 4)
+@pytest.mark.parametrize("nt", [3, 4])
+def test_multi_species_energy_and_forces_against_numpy_definition(nt):
+    """[ti*nt + tj] indexing with nt > 2 (a 2-type test cannot tell ti*nt+tj from ti*2+tj or from tj*nt+ti on a
+    symmetric table): energy from the definition, forces from its central differences, per-pair cut-offs included."""
+    w = workloads.alloy(workloads.config(0, scale=5), 11, n_types=nt, pair_cutoffs=True)
+    rng = np.random.default_rng(3)
+    idx = rng.choice(w.n_atoms, 28, replace=False)
+    pos = w.positions[idx] * 0.57 + 20.0
+    types = w.types[idx]
+    assert len(np.unique(types)) == nt
+    kw = dict(pot_kind=0, mass=w.mass, tbsma=w.tbsma, box=np.full(3, 60.0), cutoff=4.9, skin=0.3, velocities=np.zeros((28, 3)),
+              types=types, n_boxes=1, pair_cutoff=w.pair_cutoff, pair_taper_on=w.pair_taper_on)
+    f, e, _ = Oracle(positions=pos, **kw).compute_forces()
+    eref = _alloy_energy_numpy(pos, types, w.tbsma, 4.9, w.pair_cutoff, w.pair_taper_on, nt=nt)
+    assert abs(e.sum() - eref) < 1e-12 * abs(eref)
+    h = 1e-4
+    for a, c in ((0, 0), (7, 1), (19, 2), (27, 0)):
+        def E(dh):
+            p2 = pos.copy(); p2[a, c] += dh
+            return _alloy_energy_numpy(p2, types, w.tbsma, 4.9, w.pair_cutoff, w.pair_taper_on, nt=nt)
+        fd = -((8 * (E(h) - E(-h)) - (E(2 * h) - E(-2 * h))) / (12 * h))
+        assert abs(fd - f[a, c]) < 2e-8 * max(1.0, abs(f[a, c]))
+
+
+@pytest.mark.parametrize("cfg,nt", [("0", 3), ("1", 3), ("0", 4), ("1", 4)])
+def test_multi_species_label_permutation(cfg, nt):
+    """re-labelling the species cyclically (t -> t+1 mod nt) together with every parameter block / table / mass / pair
+    cut-off changes nothing, bit for bit: catches a transposed or mis-strided type-pair index in any array."""
+    w = workloads.alloy(workloads.config(cfg, scale=5 if cfg == "0" else 7), 5, n_types=nt, pair_cutoffs=True)
+    new_of_old = (np.arange(nt) + 1) % nt
+    old_of_new = np.argsort(new_of_old)
+    pair_src = [old_of_new[s] * nt + old_of_new[t] for s in range(nt) for t in range(nt)]      # new block (s,t) <- old block
+    sw = workloads.Workload(**{**w.__dict__})
+    sw.types = new_of_old[w.types].astype(np.int32)
+    sw.mass = w.mass[old_of_new].copy()
+    sw.pair_cutoff = w.pair_cutoff[pair_src].copy()
+    if cfg == "0":
+        sw.tbsma = {k: (w.tbsma[k][pair_src].copy() if k != "taper_on" else w.tbsma[k]) for k in w.tbsma}
+        sw.pair_taper_on = w.pair_taper_on[pair_src].copy()
+    else:
+        t, nr, nrho = w.tables, w.tables["nr"], w.tables["nrho"]
+        blk = lambda a, n, order: np.concatenate([a[i * n:(i + 1) * n] for i in order])
+        sw.tables = {**t, **{k: blk(t[k], nr, pair_src) for k in ("f_val", "f_der", "phi_val", "phi_der")},
+                     **{k: blk(t[k], nrho, old_of_new) for k in ("F_val", "F_der")}}
+    fa, ea, va = Oracle(w).compute_forces()
+    fb, eb, vb = Oracle(sw).compute_forces()
+    assert np.array_equal(fa, fb) and np.array_equal(ea, eb) and np.array_equal(va, vb)
+    one = workloads.config(cfg, scale=5 if cfg == "0" else 7)
+    assert not np.allclose(fa, Oracle(one).compute_forces()[0], atol=1e-3)
+    assert np.abs(fa.sum(0)).max() < 1e-11
+    oa, ob = Oracle(w), Oracle(sw)
+    oa.step(15, w.dt); ob.step(15, w.dt)
+    assert np.array_equal(oa.positions(), ob.positions())                      # masses follow the labels too
+
+
+# ---------------------------------------------------------------- F(rho) above the last table node (reading A8)
+def test_embedding_linear_continuation_above_rho_max(pins):
+    """rho >= rho_max: F = F(rho_max) + F'(rho_max)(rho - rho_max), F' = F'(rho_max).  Fe-form EAM tabulated only up to
+    rho_max = 8 while the perfect bcc lattice has rho = 10.76: closed form from tests/golden/make_lattice_pins.py."""
+    w = workloads.bcc_eam(6, 2.855, 2.4725, 5.0, "Fe", sigma=0.0, temperature=0.0, rho_max=8.0)
+    o = Oracle(w)
+    f, e, vir = o.compute_forces()
+    rho, fp = o.densities()
+    assert np.abs(rho - pins["fe.rho"]).max() < 1e-11 and rho.min() > 8.0
+    assert np.abs(e - pins["fe_rhomax8.E"]).max() < 1e-11
+    assert np.abs(fp - pins["fe_rhomax8.Fp"]).max() < 1e-15
+    assert abs(vir[0, :3].sum() / w.n_atoms - pins["fe_rhomax8.W"]) < 2e-8
+    assert np.abs(f).max() < 1e-12
+    # the two branches join continuously and forces stay the gradient of the energy across the junction: a jittered
+    # crystal whose densities straddle rho_max
+    wj = workloads.bcc_eam(6, 2.855, 2.4725, 5.0, "Fe", sigma=0.05, temperature=0.0, rho_max=10.76, seed=77)
+    oj = Oracle(wj)
+    fj, ej, _ = oj.compute_forces()
+    rj = oj.densities()[0]
+    assert (rj > 10.76).sum() > 20 and (rj < 10.76).sum() > 20
+    h = 1e-4
+    for a, c in ((3, 0), (100, 1), (211, 2)):
+        def E(dh):
+            p2 = wj.positions.copy(); p2[a, c] += dh
+            return Oracle(wj, positions=p2).compute_forces()[1].sum()
+        fd = -((8 * (E(h) - E(-h)) - (E(2 * h) - E(-2 * h))) / (12 * h))
+        assert abs(fd - fj[a, c]) < 5e-8 * max(1.0, abs(fj[a, c]))
+
+
+# ---------------------------------------------------------------- the oracle under the sanitizers (SURVEY.md section 5)
+def test_oracle_under_address_and_undefined_sanitizers(tmp_path):
+    """eam_oracle.c compiled with -fsanitize=address,undefined and driven from a small C main over both potential
+    kinds, batched boxes, rebuilds and the getters: no heap error, no undefined behaviour."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = str(tmp_path / "oracle_asan")
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fsanitize=address,undefined",
+           "-fno-sanitize-recover=undefined", "-I", os.path.join(root, "oracle"), os.path.join(root, "tests", "oracle_asan_main.c"),
+           os.path.join(root, "oracle", "eam_oracle.c"), "-lm", "-o", exe]
+    subprocess.run(cmd, check=True)
+    env = {**os.environ, "ASAN_OPTIONS": "detect_leaks=1:abort_on_error=0", "OMP_NUM_THREADS": "2"}
+    r = subprocess.run([exe], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr and "LeakSanitizer" not in r.stderr
+    assert "asan-main ok" in r.stdout

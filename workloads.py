@@ -163,7 +163,7 @@ def cu_fcc(ncell: int, cutoff: float = 4.9, skin: float = 0.3, sigma: float = 0.
 
 def bcc_eam(ncell: int, a: float, re: float, cutoff: float, element: str, skin: float = 0.3, sigma: float = 0.05,
             temperature: float = 600.0, seed: int = BASE_SEED, dt: float = 1.0, steps: int = 1000,
-            pka_ev: float = 0.0, taper_width: float = 0.0, name: str | None = None) -> Workload:
+            pka_ev: float = 0.0, taper_width: float = 0.0, name: str | None = None, rho_max: float = 100.0) -> Workload:
     """bcc crystal with the tabulated analytic EAM; optional primary knock-on atom (PKA):
     the atom nearest the box centre (lowest index on ties) has its velocity REPLACED by
     sqrt(2 E/m) along a seeded isotropic direction, after the centre-of-mass step."""
@@ -184,7 +184,7 @@ def bcc_eam(ncell: int, a: float, re: float, cutoff: float, element: str, skin: 
     return Workload(name=name or f"{element}_bcc_{ncell}^3_rc{cutoff}", box=np.full(3, a * ncell), positions=pos,
                     velocities=vel, types=np.zeros(n, dtype=np.int32), mass=np.array([MASS_AMU[element]]),
                     cutoff=cutoff, skin=skin, n_boxes=1, pot_kind=1,
-                    tables=eam_tables(re, cutoff, taper_width=taper_width), dt=dt, steps=steps, meta=meta)
+                    tables=eam_tables(re, cutoff, taper_width=taper_width, rho_max=rho_max), dt=dt, steps=steps, meta=meta)
 
 
 # --------------------------------------------------------------------------------------
@@ -222,38 +222,88 @@ def config(k: int | str, scale: int | None = None, replica: int = 0) -> Workload
     raise ValueError(f"unknown config {k!r}")
 
 
-def alloy(w: Workload, seed: int, fraction: float = 0.5, pair_cutoffs: bool = False) -> Workload:
-    """Binary alloy on the sites of `w` (the paper's rho^(ab), V^(ab)):
-    a seeded `fraction` of the atoms becomes type 1.  TB-SMA: type 1 gets a second, synthetic parameter set (larger
-    atom, different stiffness) and the cross pair (0,1) = (1,0) its own set, so that every entry of the 2x2 parameter
-    arrays differs; tables: the three pair tables are the analytic EAM with different (re, beta, A, B) and the two
-    embedding tables differ in F0.  Parameter arrays are indexed [ti * n_types + tj].  `pair_cutoffs`: the three
-    pairs also get their own cut-offs (r_c, 0.93 r_c, 0.97 r_c; TB-SMA: each switch over its last 0.5 A)."""
+def _tbsma_type_set(a: dict, s: float) -> dict:
+    """synthetic TB-SMA parameter set of a type at fraction s in [0, 1] between the base element (s = 0) and the
+    larger, stiffer synthetic element of the binary alloy (s = 1)"""
+    return dict(A=(1 + 0.2 * s) * a["A"], xi=(1 - 0.04 * s) * a["xi"], p=(1 - 0.003 * s) * a["p"], q=(1 + 0.38 * s) * a["q"],
+                r0=(1 + 0.06 * s) * a["r0"])
+
+
+def alloy(w: Workload, seed: int, fraction: float = 0.5, pair_cutoffs: bool = False, n_types: int = 2) -> Workload:
+    """Alloy on the sites of `w` (the paper's rho^(ab), V^(ab)).
+    n_types = 2: a seeded `fraction` of the atoms becomes type 1.  TB-SMA: type 1 gets a second, synthetic parameter
+    set (larger atom, different stiffness) and the cross pair (0,1) = (1,0) its own set, so that every entry of the 2x2
+    parameter arrays differs; tables: the three pair tables are the analytic EAM with different (re, beta, A, B) and the
+    two embedding tables differ in F0.  n_types = 3, 4 (MD_MAX_TYPES): equal seeded fractions; type t sits at
+    s_t = t/(n_types-1) between the two elements of the binary alloy, a cross pair (s,t) takes the mean of its two types
+    times a factor that is symmetric in (s,t) and different for every unordered pair, so every one of the
+    n_types(n_types+1)/2 parameter sets / tables differs; masses 1, 1.7, 1.3, 2.1 x the base mass.
+    Parameter arrays are indexed [ti * n_types + tj].  `pair_cutoffs`: every unordered pair also gets its own cut-off
+    in [0.93 r_c, r_c] (pair (0,0) keeps r_c; TB-SMA: each switch over its last 0.5 A)."""
     rng = np.random.Generator(np.random.PCG64(seed))
-    types = (rng.random(w.n_atoms) < fraction).astype(np.int32)
+    u = rng.random(w.n_atoms)
+    nt = int(n_types)
+    types = (u < fraction).astype(np.int32) if nt == 2 else np.minimum((u * nt).astype(np.int32), nt - 1)
     w2 = Workload(**{**w.__dict__})
     w2.types = types
-    w2.mass = np.array([w.mass[0], 1.7 * w.mass[0]])
-    w2.name = w.name + "_alloy"
+    w2.mass = w.mass[0] * np.array([1.0, 1.7, 1.3, 2.1][:nt])
+    w2.name = w.name + ("_alloy" if nt == 2 else f"_alloy{nt}")
+    pairs = [(s, t) for s in range(nt) for t in range(nt)]
+    cross = lambda s, t: 1.0 + 0.011 * (s + t) + 0.006 * s * t                 # symmetric, distinct per unordered pair
     if w.pot_kind == 0:
         a = {k: float(w.tbsma[k][0]) for k in ("A", "xi", "p", "q", "r0")}
-        b = dict(A=1.2 * a["A"], xi=0.96 * a["xi"], p=0.997 * a["p"], q=1.38 * a["q"], r0=1.06 * a["r0"])     # type 1
-        c = dict(A=1.09 * a["A"], xi=0.985 * a["xi"], p=1.01 * a["p"], q=1.17 * a["q"], r0=1.03 * a["r0"])    # cross
-        w2.tbsma = {k: np.array([a[k], c[k], c[k], b[k]]) for k in a}
+        if nt == 2:
+            b = dict(A=1.2 * a["A"], xi=0.96 * a["xi"], p=0.997 * a["p"], q=1.38 * a["q"], r0=1.06 * a["r0"])     # type 1
+            c = dict(A=1.09 * a["A"], xi=0.985 * a["xi"], p=1.01 * a["p"], q=1.17 * a["q"], r0=1.03 * a["r0"])    # cross
+            w2.tbsma = {k: np.array([a[k], c[k], c[k], b[k]]) for k in a}
+        else:
+            sets = [_tbsma_type_set(a, t / (nt - 1)) for t in range(nt)]
+
+            def entry(k, s, t):
+                if s == t:
+                    return sets[s][k]
+                mean = 0.5 * (sets[s][k] + sets[t][k])
+                return mean * cross(s, t) if k in ("A", "q") else mean / cross(s, t) if k == "xi" else mean
+            w2.tbsma = {k: np.array([entry(k, s, t) for s, t in pairs]) for k in a}
         w2.tbsma["taper_on"] = w.tbsma["taper_on"]
     else:
-        t = w.tables
+        t0 = w.tables
         re = w.meta.get("re", 2.4725)
-        rc = t["dr"] * (t["nr"] - 1)
-        t11 = eam_tables(1.05 * re, rc, nr=t["nr"], nrho=t["nrho"], beta=5.5, A=0.45, B=0.62, F0=2.9)
-        t01 = eam_tables(1.02 * re, rc, nr=t["nr"], nrho=t["nrho"], beta=5.8, A=0.42, B=0.61)
-        pair = lambda k: np.concatenate([t[k], t01[k], t01[k], t11[k]])
-        w2.tables = dict(nr=t["nr"], dr=t["dr"], nrho=t["nrho"], drho=t["drho"],
+        rc = t0["dr"] * (t0["nr"] - 1)
+        rho_max = t0["drho"] * (t0["nrho"] - 1)
+
+        def mk(re, **kw):
+            return eam_tables(re, rc, nr=t0["nr"], nrho=t0["nrho"], rho_max=rho_max, **kw)
+        if nt == 2:
+            t11 = mk(re=1.05 * re, beta=5.5, A=0.45, B=0.62, F0=2.9)
+            t01 = mk(re=1.02 * re, beta=5.8, A=0.42, B=0.61)
+            tabs = {(0, 0): t0, (0, 1): t01, (1, 0): t01, (1, 1): t11}
+        else:
+            par = lambda s: dict(re=(1 + 0.05 * s) * re, beta=6.0 - 0.5 * s, A=0.4 + 0.05 * s, B=0.6 + 0.02 * s, F0=2.5 + 0.4 * s)
+            tabs = {}
+            for s, t in pairs:
+                if (t, s) in tabs:
+                    tabs[(s, t)] = tabs[(t, s)]
+                elif s == t:
+                    tabs[(s, t)] = t0 if s == 0 else mk(**par(s / (nt - 1)))
+                else:
+                    ps, pt = par(s / (nt - 1)), par(t / (nt - 1))
+                    m = {k: 0.5 * (ps[k] + pt[k]) for k in ps}
+                    tabs[(s, t)] = mk(re=m["re"], beta=m["beta"] / cross(s, t), A=m["A"] * cross(s, t), B=m["B"])
+        pair = lambda k: np.concatenate([tabs[st][k] for st in pairs])
+        w2.tables = dict(nr=t0["nr"], dr=t0["dr"], nrho=t0["nrho"], drho=t0["drho"],
                          f_val=pair("f_val"), f_der=pair("f_der"), phi_val=pair("phi_val"), phi_der=pair("phi_der"),
-                         F_val=np.concatenate([t["F_val"], t11["F_val"]]), F_der=np.concatenate([t["F_der"], t11["F_der"]]))
+                         F_val=np.concatenate([tabs[(t, t)]["F_val"] for t in range(nt)]),
+                         F_der=np.concatenate([tabs[(t, t)]["F_der"] for t in range(nt)]))
     if pair_cutoffs:
         rc = w.cutoff
-        w2.pair_cutoff = np.array([rc, 0.93 * rc, 0.93 * rc, 0.97 * rc])
+        if nt == 2:
+            w2.pair_cutoff = np.array([rc, 0.93 * rc, 0.93 * rc, 0.97 * rc])
+        else:
+            # unordered pair number u = 0 .. n(n+1)/2 - 1 in the order (0,0), (0,1), ...: cut-offs spread over [0.93 r_c, r_c]
+            order = {st: k for k, st in enumerate((s, t) for s in range(nt) for t in range(s, nt))}
+            npair = len(order)
+            w2.pair_cutoff = np.array([rc * (1.0 - 0.07 * ((order[(min(s, t), max(s, t))] * 7) % npair) / (npair - 1)) for s, t in pairs])
         if w.pot_kind == 0:
             w2.pair_taper_on = w2.pair_cutoff - 0.5
         w2.name += "_rcut"
