@@ -15,7 +15,10 @@ Keys beyond the base contract:
                 ("bound": "alu"); `hbm` inside it gives the same kernel's algorithmic bytes / duration
                 against MEASURED_PEAKS.json's copy bandwidth.  Per-unit figures: DESIGN.md section 7.
   kernels       device time per kernel class over a separately profiled run of the same K steps.
-  cpu_baseline  the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+                `frac_survey_units` repeats it with SURVEY.md section 8(d)'s pre-kernel estimate of the work and
+                `frac_executed` with the FP64 instructions the kernel EXECUTES (ncu counters of the committed capture,
+                profiles/ncu_<workload>.json, used only while csrc/ still hashes to the capture's sources).
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on the IDENTICAL full-size input: all host cores, and one thread.
   e2e           the same metric with HOST buffers: every step copies positions and velocities host->device
                 (pinned), runs md_step(1), and copies them back.
 Multi-GPU (--gpus N under torchrun): replicas only — one independent system per GPU, no collective on the
@@ -43,32 +46,49 @@ UNIT = "atom-steps/s"
 
 # Perfect-lattice pair counts (SURVEY.md section 8 geometry table): in-cutoff neighbours per atom.
 IN_CUTOFF = {"0": 42, "1": 58, "2": 42, "3a": 42, "3": 42, "3b": 86, "4": 58}
-# bounded oracle sample: unit cells per edge (boxes for config 2) of the reduced system of the same kind
-SAMPLE_SCALE = {"0": 6, "1": 24, "2": 64, "3a": 24, "3": 24, "3b": 20, "4": 24}
-
 # Algorithmic FP64-pipe instruction counts: the FP64 instructions that the formulas need per
 # pair in the best formulation known to this repo (FMA = 1), counted on USEFUL pairs only (lanes that idle in a
 # ragged warp, parked skin pairs and loop overhead are not work).  Per LISTED pair and pass: the distance test; per
 # IN-CUTOFF pair: the potential terms.  TB-SMA: rsqrt (5) + r (1) + one (density) or two (force) exp of 11 + quintic
 # switch (6 / 10) + combine; tables: rsqrt + r + index (2) + one or two cubic-Hermite polynomials + combine.
-# SURVEY.md section 8(d) estimated 13 / 45 / 95 before any kernel existed; round 1 replaced the estimate by these
-# counts, read off the SASS of the committed kernels, so that `frac` tracks ncu's FP64-pipe utilisation.
 SLOTS = {
     0: dict(dist=6, dens=25, force=48),     # MD_POT_TBSMA   (r2 with two FMAs: reading A3 only binds the list build)
     1: dict(dist=8, dens=11, force=18),     # MD_POT_EAM_TABLE (canonical r2: the strict cut-off test decides a step)
 }
+# SURVEY.md section 8(d)'s figures, estimated before any kernel existed (libm exp / sqrt, minimum image per pass):
+# printed beside the repo's own units so that `frac` cannot only go down when the kernels get leaner.
+SURVEY_SLOTS = {0: dict(dist=13, dens=45, force=95), 1: dict(dist=13, dens=25, force=60)}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two passes, from the committed `ncu --set full`
-# capture of this command on this workload (profiles/r01k_ncu_cfg3a.md); None for workloads without a capture.
-NCU_TRAFFIC = {"3a": {"force": 338.6e6, "density": 313.8e6, "fp64_pipe_active_pct": {"force": 56.4, "density": 48.4},
-                      "source": "profiles/r01k_ncu_cfg3a.md"}}
+def csrc_sha() -> str:
+    """sha256 over the CUDA sources (sorted by name): the key that ties an ncu capture to the kernels it profiled."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1212_6332_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
 
 
-def algorithmic(kind: int, n_atoms: int, list_entries: float, in_cutoff: float) -> dict:
+def ncu_capture(workload: str) -> dict | None:
+    """Counters of the committed `ncu --set full` capture of this workload's two passes (profiles/ncu_<workload>.json,
+    written by `python -m paper_1212_6332_b200.ncu_summary`), or None when the sources have changed since."""
+    try:
+        with open(os.path.join(ROOT, "profiles", f"ncu_{workload}.json")) as fh:
+            cap = json.load(fh)
+    except Exception:  # noqa: BLE001
+        return None
+    if cap.get("csrc_sha") != csrc_sha():
+        return {"stale": True, "source": cap.get("source"), "csrc_sha_of_capture": cap.get("csrc_sha")}
+    return cap
+
+
+def algorithmic(kind: int, n_atoms: int, list_entries: float, in_cutoff: float, units: dict = SLOTS) -> dict:
     """Algorithmic work of ONE force-pass launch and ONE density-pass launch."""
     m = list_entries / n_atoms
-    s = SLOTS[kind]
+    s = units[kind]
     return dict(
         force_slots=n_atoms * (m * s["dist"] + in_cutoff * s["force"]),
         dens_slots=n_atoms * (m * s["dist"] + in_cutoff * s["dens"]),
@@ -137,32 +157,40 @@ def measured_peaks() -> tuple[float, str]:
 # --------------------------------------------------------------------------------------------------------
 # the CPU oracle: cpu_baseline leg and --impl reference arm
 # --------------------------------------------------------------------------------------------------------
-def oracle_sample(workload: str):
+def oracle_full(workload: str, threads: int = 0):
+    """The oracle on the IDENTICAL input the CUDA arm times (full size, replica 0)."""
     from oracle import Oracle, set_threads
-    cores = set_threads(0)
-    w = workloads.config(workload, scale=SAMPLE_SCALE[workload])
+    cores = set_threads(threads)
+    w = workloads.config(workload)
     return Oracle(w), w, cores
 
 
 def time_oracle(workload: str, budget_s: float) -> dict:
-    """atom-steps/s of the oracle on a bounded sample; about `budget_s` seconds of wall time."""
-    o, w, cores = oracle_sample(workload)
-    t0 = time.perf_counter()
-    o.step(1, w.dt)                       # builds the list and evaluates the initial forces: untimed warm-up
-    t_first = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    o.step(2, w.dt)
-    per = (time.perf_counter() - t0) / 2
-    n = int(max(3, min(w.steps, budget_s / max(per, 1e-6))))
-    r0 = o.stats()["rebuilds"]
-    t0 = time.perf_counter()
-    o.step(n, w.dt)
-    t = time.perf_counter() - t0
-    return {"value": w.n_atoms * n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{w.name} reduced to {w.n_atoms} atoms ({SAMPLE_SCALE[workload]} per edge), {n} steps of dt={w.dt} fs "
-                      f"incl. {o.stats()['rebuilds'] - r0} rebuilds, OpenMP over atoms, full (directed) lists; "
-                      f"first step (list build + 2 force evaluations) {t_first:.2f} s untimed",
-            "ms_per_step": 1e3 * t / n}
+    """atom-steps/s of the oracle, as it stands, on the full-size input: all host cores (up to 10 steps within about
+    `budget_s` seconds) and single-threaded (2 steps); list builds that fall into the timed steps are included."""
+    out = {}
+    for label, threads, share in (("all_cores", 0, 0.6), ("single_thread", 1, 0.4)):
+        o, w, cores = oracle_full(workload, threads)
+        t0 = time.perf_counter()
+        o.step(1, w.dt)                   # builds the list and evaluates the initial forces: untimed warm-up
+        t_first = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        o.step(1, w.dt)
+        per = time.perf_counter() - t0
+        n = int(max(1, min(10 if threads == 0 else 2, share * budget_s / max(per, 1e-6))))
+        r0 = o.stats()["rebuilds"]
+        t0 = time.perf_counter()
+        o.step(n, w.dt)
+        t = time.perf_counter() - t0
+        out[label] = {"value": w.n_atoms * n / t, "cores": cores, "steps": n, "ms_per_step": 1e3 * t / n,
+                      "rebuilds": o.stats()["rebuilds"] - r0, "first_step_s": round(t_first, 2)}
+        del o
+    a = out["all_cores"]
+    return {"value": a["value"], "unit": UNIT, "cores": a["cores"], "kind": "oracle",
+            "sample": f"{full_name(workload)}: the identical full-size input ({w.n_atoms} atoms), {a['steps']} steps of dt={w.dt} fs "
+                      f"incl. {a['rebuilds']} rebuilds, OpenMP over atoms on {a['cores']} threads, full (directed) lists; the first step "
+                      f"(list build + 2 force evaluations, {a['first_step_s']} s) untimed",
+            "ms_per_step": a["ms_per_step"], "single_thread": out["single_thread"]}
 
 
 def whole_job_value(ms_local: float, n_atoms_per_rank: int, steps: int, world: int, device: str = "cuda") -> tuple[float, float]:
@@ -181,18 +209,18 @@ def whole_job_value(ms_local: float, n_atoms_per_rank: int, steps: int, world: i
 def reference_arm(args, rank: int):
     if rank != 0:
         return
-    o, w, cores = oracle_sample(args.workload)
+    o, w, cores = oracle_full(args.workload)
     o.step(max(args.warmup, 1), w.dt)
     t0 = time.perf_counter()
     o.step(args.steps, w.dt)
     t = time.perf_counter() - t0
     value = w.n_atoms * args.steps / t
-    sample = (f"{w.name} reduced to {w.n_atoms} atoms ({SAMPLE_SCALE[args.workload]} per edge); every step is one "
-              f"oracle_step of that sample on the host cores")
+    sample = (f"{w.name}: the identical full-size input ({w.n_atoms} atoms); every step is one oracle_step on {cores} host threads")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": full_name(args.workload), "sample_atoms": w.n_atoms},
+            "config": {"workload": full_name(args.workload), "n_atoms_per_gpu": w.n_atoms, "n_boxes": w.n_boxes, "cutoff": w.cutoff,
+                       "skin": w.skin, "dt_fs": w.dt},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -266,22 +294,37 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
     dfma_rate, dfma_mhz = md.fp64_dfma_rate()
     hbm_peak, hbm_src = measured_peaks()
     alg = algorithmic(w.pot_kind, w.n_atoms, st2["list_entries"], IN_CUTOFF[args.workload])
+    alg_s = algorithmic(w.pot_kind, w.n_atoms, st2["list_entries"], IN_CUTOFF[args.workload], SURVEY_SLOTS)
     f_ms = prof["force"][1] / prof["force"][0]
     d_ms = prof["density"][1] / prof["density"][0]
+    cap = ncu_capture(args.workload) if args.scale is None else None
+    live = cap is not None and not cap.get("stale")
+    cf, cd = (cap["kernels"]["force"], cap["kernels"]["density"]) if live else ({}, {})
+
+    def executed(c, ms):          # FP64 thread-instructions the kernel executed (ncu, per launch) / this run's duration / the peak
+        return c["fp64_thread_inst"] / (ms * 1e-3) / dfma_rate if c.get("fp64_thread_inst") else None
+
     roofline = {
-        "kernel": "k_force (force pass + fused second half-kick)", "bound": "alu",
+        "kernel": "k_force (force pass + fused half-kicks and drift)", "bound": "alu",
         "achieved": alg["force_slots"] / (f_ms * 1e-3) / 1e12, "peak": dfma_rate / 1e12, "unit": "T FP64-inst/s",
         "frac": alg["force_slots"] / (f_ms * 1e-3) / dfma_rate,
-        "traffic": NCU_TRAFFIC.get(args.workload, {}).get("force") if args.scale is None else None,
-        "ncu": NCU_TRAFFIC.get(args.workload) if args.scale is None else None,
+        "frac_survey_units": alg_s["force_slots"] / (f_ms * 1e-3) / dfma_rate,
+        "frac_executed": executed(cf, f_ms),
+        "useful_over_executed": alg["force_slots"] / cf["fp64_thread_inst"] if cf.get("fp64_thread_inst") else None,
+        "traffic": cf.get("dram_bytes"),
+        "ncu": cap,
         "peak_source": f"md_fp64_dfma_rate measured in this run at {dfma_mhz:.0f} MHz",
         "ms_per_launch": f_ms, "algorithmic_fp64_inst_per_launch": alg["force_slots"],
+        "survey_fp64_inst_per_launch": alg_s["force_slots"],
+        "units": {"repo": SLOTS[w.pot_kind], "survey": SURVEY_SLOTS[w.pot_kind], "in_cutoff_pairs_per_atom": IN_CUTOFF[args.workload]},
         "hbm": {"achieved": alg["force_bytes"] / (f_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": alg["force_bytes"] / (f_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "algorithmic_bytes_per_launch": alg["force_bytes"]},
         "density": {"ms_per_launch": d_ms, "achieved": alg["dens_slots"] / (d_ms * 1e-3) / 1e12,
                     "frac": alg["dens_slots"] / (d_ms * 1e-3) / dfma_rate,
-                    "hbm_frac": alg["dens_bytes"] / (d_ms * 1e-3) / 1e9 / hbm_peak},
+                    "frac_survey_units": alg_s["dens_slots"] / (d_ms * 1e-3) / dfma_rate,
+                    "frac_executed": executed(cd, d_ms),
+                    "hbm_frac": alg["dens_bytes"] / (d_ms * 1e-3) / 1e9 / hbm_peak, "traffic": cd.get("dram_bytes")},
     }
 
     # ---- end to end with HOST buffers: H2D of x and v, one step, D2H of x and v, every step --------------
@@ -329,7 +372,7 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
                        "l2": f"no flush: per-step working set (neighbour list {4 * st2['list_entries'] / 2 ** 20:.0f} MiB + per-atom "
                              f"arrays, workspace {ws_mb:.0f} MiB) exceeds the 126 MB L2" if 4 * st2["list_entries"] > 126e6
                              else "no flush: working set fits L2 (small config; steady-state MD keeps it there by design)"},
-            "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
+            "clocks": clocks, "gpu_launches": launches, "graph_active": st1["graph_active"], "e2e": e2e, "roofline": roofline, "kernels": kernels,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)

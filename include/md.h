@@ -105,7 +105,7 @@ typedef struct {
   int neighbor_capacity;          /* list capacity per atom in use */
   long kernel_launches;           /* CUDA kernels this system has enqueued since md_create (host-side count) */
   long list_entries;              /* sum over atoms of the list lengths of the last build (directed pairs) */
-  int graph_active;               /* 1: the last md_step replayed the CUDA graph of one step (MD_OPT_GRAPH); 0: plain launches */
+  int graph_active;               /* 1: the last md_step replayed its CUDA graphs (MD_OPT_GRAPH); 0: plain launches */
   int graph_error;                /* cudaError_t of a failed graph build (0: none).  md_step then runs the same kernels as
                                      plain launches for the life of the system (or until MD_OPT_GRAPH is set to 1 again) */
 } md_stats;
@@ -176,12 +176,15 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                              (the paper's full-MD runs).  md_compute_forces always computes them.
  *  MD_OPT_PROFILE           1: bracket every kernel launch with CUDA events on the system's stream so that
  *                              md_profile_read can report per-kernel device time.
- *  MD_OPT_FORCE_VARIANT     0: choose by system size (8 lanes per atom up to 24,576 atoms); 1: one thread per atom;
- *                           2: 8 lanes per atom.
- *  MD_OPT_GRAPH             1 (default): md_step replays one CUDA graph per time step whose neighbour rebuild is
- *                           the body of a conditional node (4 kernel launches per step when no rebuild is due);
- *                           0: plain launches (every kernel of the rebuild chain is launched and returns at once
- *                           unless a rebuild is due).  MD_OPT_PROFILE implies plain launches. */
+ *  MD_OPT_FORCE_VARIANT     lanes per atom in the two passes.  0: chosen by system size (32 lanes up to 4,096 atoms,
+ *                           8 lanes up to 24,576 atoms, else one thread per atom); 1: one thread per atom; 2: 8 lanes;
+ *                           3: 32 lanes (MD_EINVAL above 32,768 atoms); 4: 4 lanes.
+ *  MD_OPT_GRAPH             1 (default): md_step replays CUDA graphs of up to 8 time steps each; the neighbour rebuild
+ *                           of every step is the body of a conditional node, the force pass of a step also performs
+ *                           the next step's first half-kick, drift and displacement check, and the last block of that
+ *                           kernel takes the rebuild decision (2 kernel launches per step when no rebuild is due);
+ *                           0: the same kernels as plain launches (every kernel of the rebuild chain is launched and
+ *                           returns at once unless a rebuild is due).  MD_OPT_PROFILE implies plain launches. */
 enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3, MD_OPT_GRAPH = 4 };
 int md_set_option(md_system *s, int option, int value);
 

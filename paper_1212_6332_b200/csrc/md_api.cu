@@ -92,7 +92,8 @@ static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
   if (g.cap > 0xfff0) return MD_EINVAL;               // ncount packs two 16-bit counts
   g.cap = (g.cap + 3) & ~3;
   g.tiles_per_box = (g.npb + 31) / 32;
-  g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock / 8);   // block partials: enough for the 8-lanes-per-atom variant
+  // block partials: enough for the 8-lanes-per-atom variant, and for 32 lanes per atom where that variant is allowed
+  g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock / (d->n_atoms <= kSub32Limit ? 32 : 8));
   g.stage_bytes = (size_t)d->n_atoms * 3 * sizeof(double);
   if (g.stage_bytes < (1u << 20)) g.stage_bytes = 1u << 20;
   return MD_OK;
@@ -298,18 +299,25 @@ static int query_restore(md_system *s, bool stashed) {
 }
 
 static void drop_step_graph(md_system *s) {
-  if (s->step_exec) cudaGraphExecDestroy(s->step_exec);
-  if (s->step_graph) cudaGraphDestroy(s->step_graph);
-  s->step_exec = nullptr; s->step_graph = nullptr;
+  for (auto &g : s->sg) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g.exec = nullptr; g.graph = nullptr; g.nsteps = 0;
+  }
 }
 
-// One time step as a CUDA graph (built once per (dt, observables), replayed by md_step):
-//   k_kick_drift -> k_decide -> IF(do_rebuild){ clear, bin, 3 x scan, scatter, cell order, re-order, copy back, list } -> k_density -> k_force [-> k_reduce_boxes]
-// The rebuild decision stays on the device (k_decide sets the conditional node's handle), so md_step never
-// synchronises, and a step without a rebuild launches 4 kernels instead of 14.
-static int build_step_graph(md_system *s, double dt, bool obs) {
-  if (s->step_exec && s->step_dt == dt && s->step_obs == obs) return MD_OK;
-  drop_step_graph(s);
+// `nsteps` time steps as ONE CUDA graph (built once per (dt, observables, nsteps), replayed by md_step):
+//   k_kick_drift -> { IF(do_rebuild){ clear, bin, 3 x scan, scatter, cell order, re-order, copy back, list } -> k_density -> k_force [-> k_reduce_boxes] } x nsteps
+// The force pass of every step but the last also performs the next step's first half-kick, drift and displacement
+// check (StepCtl::chain), and the last block of the kernel that ends a drift takes the rebuild decision and sets the
+// handle of the following conditional node: a step without a rebuild is two kernel launches, the host never
+// synchronises, and the launch latency of a small system is paid once per graph instead of once per step.
+// With a barostat (scaling between the steps) nsteps is 1 and nothing is chained.
+static int build_step_graph(md_system *s, md_system::StepGraph &sg, double dt, bool obs, int nsteps) {
+  if (sg.exec && sg.dt == dt && sg.obs == obs && sg.nsteps == nsteps) return MD_OK;
+  if (sg.exec) cudaGraphExecDestroy(sg.exec);
+  if (sg.graph) cudaGraphDestroy(sg.graph);
+  sg.exec = nullptr; sg.graph = nullptr; sg.nsteps = 0;
   const long launches0 = s->launches;
   // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot capture);
   // nothing executes during capture, and the graph is launched on the caller's stream
@@ -321,32 +329,37 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
   }
   s->stream = st;
   cudaGraph_t g = nullptr;
-  cudaGraphConditionalHandle cond;
-  bool ok = cudaGraphCreate(&g, 0) == cudaSuccess &&
-            cudaGraphConditionalHandleCreate(&cond, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+  std::vector<cudaGraphConditionalHandle> cond((size_t)nsteps);
+  bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
+  for (int k = 0; ok && k < nsteps; ++k) ok = cudaGraphConditionalHandleCreate(&cond[k], g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
   const cudaGraphNode_t *deps = nullptr;
   size_t ndeps = 0;
   cudaGraphNode_t last = nullptr, cnode = nullptr;
   cudaGraph_t tmp = nullptr;
-  long head = 0, body = 0, tail = 0;
-  if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
-  if (ok) {
-    long l0 = s->launches;
-    ok = launch_kick_drift(s, dt) == 0 && launch_decide(s, cond, true) == 0;
-    head = s->launches - l0;
+  long fixed = 0, body = 0;
+  // the node the stream's next captured work would depend on; ends the capture
+  auto end_capture = [&](bool okin) {
+    bool o = okin;
     cudaStreamCaptureStatus cs;
 #if CUDART_VERSION >= 13000
-    if (ok) ok = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, nullptr, &ndeps) == cudaSuccess && ndeps == 1;   // + edge data
+    if (o) o = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, nullptr, &ndeps) == cudaSuccess && ndeps == 1;   // + edge data
 #else
-    if (ok) ok = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, &ndeps) == cudaSuccess && ndeps == 1;
+    if (o) o = cudaStreamGetCaptureInfo(st, &cs, nullptr, nullptr, &deps, &ndeps) == cudaSuccess && ndeps == 1;
 #endif
-    if (ok) last = deps[0];
-    ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
-  }
+    if (o) last = deps[0];
+    return (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && o;
+  };
+  if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
   if (ok) {
+    const long l0 = s->launches;
+    ok = launch_kick_drift(s, dt, make_ctl(s, dt, cond[0], true, false)) == 0;
+    fixed += s->launches - l0;
+    ok = end_capture(ok);
+  }
+  for (int k = 0; ok && k < nsteps; ++k) {
     cudaGraphNodeParams cp = {};
     cp.type = cudaGraphNodeTypeConditional;
-    cp.conditional.handle = cond;
+    cp.conditional.handle = cond[k];
     cp.conditional.type = cudaGraphCondTypeIf;
     cp.conditional.size = 1;
 #if CUDART_VERSION >= 13000
@@ -358,20 +371,22 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
       cudaGraph_t bodyg = cp.conditional.phGraph_out[0];
       ok = cudaStreamBeginCaptureToGraph(st, bodyg, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
       if (ok) {
-        long l0 = s->launches;
+        const long l0 = s->launches;
         ok = launch_rebuild_body(s) == 0;
         body = s->launches - l0;
         ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
       }
     }
-  }
-  if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, &cnode, nullptr, 1, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
-  if (ok) {
-    long l0 = s->launches;
-    ok = launch_density(s) == 0 && launch_force(s, obs, 0.5 * dt) == 0;
-    if (ok && s->baro_tau > 0.0) ok = launch_barostat(s, dt) == 0;
-    tail = s->launches - l0;
-    ok = (cudaStreamEndCapture(st, &tmp) == cudaSuccess) && ok;
+    if (ok) ok = cudaStreamBeginCaptureToGraph(st, g, &cnode, nullptr, 1, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+      const long l0 = s->launches;
+      const bool chain = k + 1 < nsteps;
+      const StepCtl ctl = make_ctl(s, dt, chain ? cond[k + 1] : cond[k], chain, chain);
+      ok = launch_density(s) == 0 && launch_force(s, obs, 0.5 * dt, &ctl) == 0;
+      if (ok && s->baro_tau > 0.0) ok = launch_barostat(s, dt) == 0;
+      fixed += s->launches - l0;
+      ok = end_capture(ok);
+    }
   }
   cudaGraphExec_t exec = nullptr;
   if (ok) ok = cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
@@ -383,13 +398,13 @@ static int build_step_graph(md_system *s, double dt, bool obs) {
     // visible to the caller as md_stats.graph_error != 0 and md_stats.graph_active == 0
     const cudaError_t err = cudaGetLastError();
     s->graph_error = err != cudaSuccess ? (int)err : (int)cudaErrorUnknown;
-    if (getenv("MD_DEBUG")) fprintf(stderr, "md: step graph unavailable (%s; head %ld body %ld tail %ld, deps %zu)\n", cudaGetErrorString(err), head, body, tail, ndeps);
+    if (getenv("MD_DEBUG")) fprintf(stderr, "md: step graph unavailable (%s; %d steps, fixed %ld body %ld, deps %zu)\n", cudaGetErrorString(err), nsteps, fixed, body, ndeps);
     if (g) cudaGraphDestroy(g);
     s->opt_graph = false;
     return MD_ECUDA;
   }
-  s->step_graph = g; s->step_exec = exec; s->step_dt = dt; s->step_obs = obs;
-  s->step_kernels = (int)(head + tail); s->body_kernels = (int)body;
+  sg.graph = g; sg.exec = exec; sg.dt = dt; sg.obs = obs; sg.nsteps = nsteps; sg.kernels = (int)fixed;
+  s->body_kernels = (int)body;
   return MD_OK;
 }
 
@@ -454,7 +469,8 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->have_list = s->forces_valid = s->observables_valid = false;
   s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
   s->thermo_Te = 0.0; s->thermo_tau = 0.0; s->baro_P0 = 0.0; s->baro_tau = 0.0;
-  s->step_graph = nullptr; s->step_exec = nullptr; s->step_dt = 0.0; s->step_obs = false; s->step_kernels = s->body_kernels = 0;
+  for (auto &g : s->sg) { g.graph = nullptr; g.exec = nullptr; g.dt = 0.0; g.obs = false; g.nsteps = 0; g.kernels = 0; }
+  s->body_kernels = 0;
   s->graph_error = 0; s->last_step_graph = false; s->frc_keep = false;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
@@ -564,7 +580,9 @@ int md_set_option(md_system *s, int option, int value) {
     case MD_OPT_STEP_OBSERVABLES: s->opt_step_obs = value != 0; return MD_OK;
     case MD_OPT_PROFILE: s->opt_profile = value != 0; return MD_OK;
     case MD_OPT_GRAPH: s->opt_graph = value != 0; if (value) s->graph_error = 0; return MD_OK;   // switching it on retries a failed build
-    case MD_OPT_FORCE_VARIANT: if (value < 0 || value > 2) return MD_EINVAL; s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
+    case MD_OPT_FORCE_VARIANT:
+      if (value < 0 || value > 4 || (value == 3 && s->d.N > kSub32Limit)) return MD_EINVAL;
+      s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
   }
   return MD_EINVAL;
 }
@@ -657,21 +675,31 @@ int md_step(md_system *s, int n, double dt) {
   if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
   const bool baro = s->baro_tau > 0.0;
   const bool obs = s->opt_step_obs || baro;          // the barostat needs the virial of every step
-  if (s->opt_graph && !s->opt_profile && build_step_graph(s, dt, obs) == MD_OK) {
-    // one graph launch per step: 4 kernels when no rebuild is due, no launch of the chain's kernels at all
-    for (int k = 0; k < n; ++k)
-      if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) return MD_ECUDA;
-    s->launches += (long)n * s->step_kernels;
+  const int unroll = baro ? 1 : kStepUnroll;         // steps per graph launch (chained: no scaling in between)
+  const int q = n / unroll, r = n % unroll;
+  cudaGraphConditionalHandle none{};
+  if (s->opt_graph && !s->opt_profile && (q == 0 || build_step_graph(s, s->sg[0], dt, obs, unroll) == MD_OK) &&
+      (r == 0 || build_step_graph(s, s->sg[1], dt, obs, r) == MD_OK)) {
+    for (int k = 0; k < q; ++k)
+      if (cudaGraphLaunch(s->sg[0].exec, s->stream) != cudaSuccess) return MD_ECUDA;
+    if (r && cudaGraphLaunch(s->sg[1].exec, s->stream) != cudaSuccess) return MD_ECUDA;
+    s->launches += (long)q * s->sg[0].kernels + (r ? s->sg[1].kernels : 0);
     s->have_list = true; s->forces_valid = true; s->observables_valid = obs && !baro;
     s->last_step_graph = true;
   } else {
+    // the same kernels in the same order as plain launches: every kernel of the rebuild chain is launched in every step
+    // and returns at once unless the decision (taken by the last block of the preceding drift) says otherwise
     s->last_step_graph = false;
-    for (int k = 0; k < n; ++k) {
-      if (launch_kick_drift(s, dt) != 0) return MD_ECUDA;
-      if ((rc = forces_sequence(s, obs, 0.5 * dt)) != MD_OK) return rc;
-      if (baro && launch_barostat(s, dt) != 0) return MD_ECUDA;
+    for (int k0 = 0; k0 < n; k0 += unroll) {
+      const int m = n - k0 < unroll ? n - k0 : unroll;
+      if (launch_kick_drift(s, dt, make_ctl(s, dt, none, false, false)) != 0) return MD_ECUDA;
+      for (int j = 0; j < m; ++j) {
+        const StepCtl ctl = make_ctl(s, dt, none, false, j + 1 < m);
+        if (launch_rebuild_body(s) != 0 || launch_density(s) != 0 || launch_force(s, obs, 0.5 * dt, &ctl) != 0) return MD_ECUDA;
+        if (baro && launch_barostat(s, dt) != 0) return MD_ECUDA;
+      }
     }
-    if (baro) s->observables_valid = false;          // energies and virial on request belong to the scaled positions
+    s->have_list = true; s->forces_valid = true; s->observables_valid = obs && !baro;   // with a barostat: energies and virial on request belong to the scaled positions
   }
   s->frc_keep = baro;
   s->steps += n;

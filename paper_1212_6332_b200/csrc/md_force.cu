@@ -583,16 +583,31 @@ __device__ __forceinline__ void force_merge(ForceAcc<OBS> &a, const ForceAcc<OBS
 
 // Epilogue of the force pass for the thread that holds the totals of atom i (valid) or nothing (!valid): store the
 // force, second half-kick, non-finite flag; OBS: per-atom energy and the block's partial sums of E and W.
+// ctl.chain: the same thread goes on with the NEXT step's first half-kick and drift (the new position goes to `pos`,
+// which this pass does not read: it gathers from `posf`) and the displacement check, so that a step inside md_step
+// costs two kernels (density, force) instead of four.
 template <bool OBS>
-__device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &kick, int i, bool valid, int ti, const ForceAcc<OBS> &acc,
-                                             double (*sm)[8]) {
+__device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &kick, const StepCtl &ctl, int i, bool valid, int ti,
+                                             const double4 &pi, const ForceAcc<OBS> &acc, double (*sm)[8], unsigned long long *smd) {
+  double d2 = 0.0;
   if (valid) {
     const size_t N = (size_t)s.N;
-    s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
     if (kick.h[ti] != 0.0) {
+      // every load of the epilogue is issued before anything waits for one of them
       double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
+      double rx = 0.0, ry = 0.0, rz = 0.0;
+      if (ctl.chain) { rx = s.xref[i]; ry = s.xref[N + i]; rz = s.xref[2 * N + i]; }
+      s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
       half_kick(kick, ti, acc.fx, acc.fy, acc.fz, vx, vy, vz);
+      if (ctl.chain) {
+        half_kick(kick, ti, acc.fx, acc.fy, acc.fz, vx, vy, vz);
+        double4 x = make_double4(pi.x, pi.y, pi.z, (double)ti);
+        d2 = drift_atom(ctl.dt, x, vx, vy, vz, rx, ry, rz);
+        s.pos[i] = x;
+      }
       s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
+    } else {
+      s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
     }
     if (!(fabs(acc.fx) + fabs(acc.fy) + fabs(acc.fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
   }
@@ -621,12 +636,14 @@ __device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &
       s.partial[(size_t)blockIdx.x * 8 + threadIdx.x] = a;
     }
   }
+  if (ctl.chain) finish_displacement(s, ctl, d2, smd);
 }
 
 template <int KIND, bool MULTI, bool OBS, bool FOLD, bool DYN>
-__global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick) {
+__global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick, const StepCtl ctl) {
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
+  __shared__ unsigned long long smd[kForceBlock / 32];
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
@@ -683,7 +700,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     if (parked) flush();
   }
 
-  force_finish<OBS>(s, kick, i, valid, ti, acc, sm);
+  force_finish<OBS>(s, kick, ctl, i, valid, ti, pi, acc, sm, smd);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -692,23 +709,31 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
 // kSub lanes of an atom take the 16-byte groups of its row round-robin and their partial sums are combined by
 // shuffles in a fixed order (deterministic).  Same arithmetic per pair as the kernels above.
 // ------------------------------------------------------------------------------------------------
-constexpr int kSub = 8, kSubAtoms = kForceBlock / kSub;
-
 struct SubMap { int box, local, i, sl; bool valid; };
+template <int SUB>
 __device__ __forceinline__ SubMap sub_map(const DevSys &s) {
+  constexpr int kSubAtoms = kForceBlock / SUB;
   SubMap m;
   const int bpb = (s.npb + kSubAtoms - 1) / kSubAtoms;
   m.box = blockIdx.x / bpb;
-  m.local = (blockIdx.x - m.box * bpb) * kSubAtoms + (threadIdx.x / kSub);
-  m.sl = threadIdx.x % kSub;
+  m.local = (blockIdx.x - m.box * bpb) * kSubAtoms + (threadIdx.x / SUB);
+  m.sl = threadIdx.x % SUB;
   m.valid = m.local < s.npb;
   m.i = m.box * s.npb + (m.valid ? m.local : 0);
   return m;
 }
 
-// calls body(entry, in_main) for the entries of the row that this sub-lane owns
-template <class Body>
+// calls body(entry, in_main) for the entries of the row that this sub-lane owns: whole 16-byte groups round-robin, or
+// (SUB >= 16: rows of a few tens of entries would leave most lanes idle) single entries round-robin
+template <int SUB, class Body>
 __device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, Body body) {
+  if constexpr (SUB >= 16) {
+    const unsigned *m = reinterpret_cast<const unsigned *>(row.main), *l = reinterpret_cast<const unsigned *>(row.last);
+    for (int k = sl; k < row.n_in; k += SUB) body(__ldg(m + nbr_entry(k)), true);
+    for (int k = sl; k < row.n_out; k += SUB) body(__ldg(l + 3 - (int)nbr_entry(k)), false);   // entry cap-1-k: group -(k>>2), component 3-(k&3)
+    return;
+  }
+  constexpr int kSub = SUB;
   for (int g = sl; g * 4 < row.n_in; g += kSub) {
     const uint4 E = ldg_group(row.main + (size_t)g * 32);
     const unsigned e[4] = {E.x, E.y, E.z, E.w};
@@ -725,18 +750,19 @@ __device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, Body body) 
   }
 }
 
-template <int KIND, bool MULTI, bool FOLD>
+template <int KIND, bool MULTI, bool FOLD, int SUB>
 __global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_constant__ DevSys s) {
+  constexpr int kSub = SUB;
   __shared__ double tab_sm[kExpTabLen];
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
-  const SubMap m = sub_map(s);
+  const SubMap m = sub_map<SUB>(s);
   const AtomRow row = atom_row(s, m.box, m.local, m.i, m.valid);
   const double4 pi = s.pos[m.i];
   const int ti = MULTI ? (int)pi.w : 0;
   double rho = 0.0;
-  walk_sub(row, m.sl, [&](unsigned e, bool in_main) {
+  walk_sub<SUB>(row, m.sl, [&](unsigned e, bool in_main) {
     const double4 pj = gather32(s.pos + MD_GIDX(e));
     double dx, dy, dz;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
@@ -756,19 +782,21 @@ __global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_consta
   s.posf[m.i] = make_double4(pi.x, pi.y, pi.z, Fp);
 }
 
-template <int KIND, bool MULTI, bool OBS, bool FOLD>
-__global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant__ DevSys s, const KickParams kick) {
+template <int KIND, bool MULTI, bool OBS, bool FOLD, int SUB>
+__global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant__ DevSys s, const KickParams kick, const StepCtl ctl) {
+  constexpr int kSub = SUB;
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
+  __shared__ unsigned long long smd[kForceBlock / 32];
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
-  const SubMap m = sub_map(s);
+  const SubMap m = sub_map<SUB>(s);
   const AtomRow row = atom_row(s, m.box, m.local, m.i, m.valid);
   const double4 pi = s.posf[m.i];
   const int ti = MULTI ? s.type[m.i] : 0;
   ForceAcc<OBS> acc;
-  walk_sub(row, m.sl, [&](unsigned e, bool in_main) {
+  walk_sub<SUB>(row, m.sl, [&](unsigned e, bool in_main) {
     const double4 pj = gather32(s.posf + MD_GIDX(e));
     double dx, dy, dz, g, V = 0.0;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
@@ -789,7 +817,7 @@ __global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant
       acc.w4 += __shfl_xor_sync(0xffffffffu, acc.w4, o); acc.w5 += __shfl_xor_sync(0xffffffffu, acc.w5, o);
     }
   }
-  force_finish<OBS>(s, kick, m.i, m.valid && m.sl == 0, ti, acc, sm);
+  force_finish<OBS>(s, kick, ctl, m.i, m.valid && m.sl == 0, ti, pi, acc, sm, smd);
 }
 
 // per box: sum the block partials in a fixed order
@@ -849,24 +877,36 @@ int launch_prepare_tables(md_system *sys) {
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-// variant of the two passes: kSub lanes per atom while one thread per atom would leave SMs idle
-bool use_sub_lanes(const md_system *sys) {
-  if (sys->opt_force_variant == 1) return false;
-  if (sys->opt_force_variant == 2) return true;
-  return sys->d.N <= kSubMaxAtoms;
+// variant of the two passes: lanes per atom.  One thread per atom fills the GPU from ~25 k atoms on; below that the
+// lanes of an atom share its row (8 lanes, or 32 for a few thousand atoms, where a step is pure latency).
+int sub_lanes(const md_system *sys) {
+  switch (sys->opt_force_variant) {
+    case 1: return 1;
+    case 2: return 8;
+    case 3: return sys->d.N <= kSub32Limit ? 32 : 8;
+    case 4: return 4;
+  }
+  if (sys->d.N <= kSub32MaxAtoms) return 32;
+  return sys->d.N <= kSubMaxAtoms ? 8 : 1;
 }
 int force_blocks(const md_system *sys) {
-  return sys->d.nb * blocks_per_box(sys->d.npb, use_sub_lanes(sys) ? kSubAtoms : kForceBlock);
+  return sys->d.nb * blocks_per_box(sys->d.npb, kForceBlock / sub_lanes(sys));
+}
+
+template <int KIND, bool FOLD, int SUB>
+static void launch_density_sub(md_system *sys, int grid) {
+  if (sys->d.nt > 1) k_density_sub<KIND, true, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+  else k_density_sub<KIND, false, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
 }
 
 template <int KIND, bool FOLD>
 static void launch_density_k(md_system *sys, int grid) {
-  if (use_sub_lanes(sys)) {
-    if (sys->d.nt > 1) ++sys->launches, k_density_sub<KIND, true, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    else ++sys->launches, k_density_sub<KIND, false, FOLD><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    return;
-  }
   ++sys->launches;
+  switch (sub_lanes(sys)) {
+    case 32: launch_density_sub<KIND, FOLD, 32>(sys, grid); return;
+    case 8: launch_density_sub<KIND, FOLD, 8>(sys, grid); return;
+    case 4: launch_density_sub<KIND, FOLD, 4>(sys, grid); return;
+  }
   if (sys->d.dyn_box) {
     if (sys->d.nt > 1) k_density<KIND, true, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
     else k_density<KIND, false, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
@@ -886,49 +926,58 @@ int launch_density(md_system *sys) {
   return (int)cudaGetLastError();
 }
 
+template <int KIND, bool FOLD, int SUB>
+static void launch_force_sub(md_system *sys, int grid, bool obs, const KickParams &kp, const StepCtl &ctl) {
+  cudaStream_t st = sys->stream;
+  if (sys->d.nt > 1) {
+    if (obs) k_force_sub<KIND, true, true, FOLD, SUB><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    else k_force_sub<KIND, true, false, FOLD, SUB><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+  } else {
+    if (obs) k_force_sub<KIND, false, true, FOLD, SUB><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    else k_force_sub<KIND, false, false, FOLD, SUB><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+  }
+}
+
 template <int KIND, bool FOLD>
-static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams &kp) {
+static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams &kp, const StepCtl &ctl) {
   const bool multi = sys->d.nt > 1;
   cudaStream_t st = sys->stream;
   ++sys->launches;
-  if (use_sub_lanes(sys)) {
-    if (multi) {
-      if (obs) k_force_sub<KIND, true, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force_sub<KIND, true, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-    } else {
-      if (obs) k_force_sub<KIND, false, true, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force_sub<KIND, false, false, FOLD><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-    }
-    return;
+  switch (sub_lanes(sys)) {
+    case 32: launch_force_sub<KIND, FOLD, 32>(sys, grid, obs, kp, ctl); return;
+    case 8: launch_force_sub<KIND, FOLD, 8>(sys, grid, obs, kp, ctl); return;
+    case 4: launch_force_sub<KIND, FOLD, 4>(sys, grid, obs, kp, ctl); return;
   }
   if (multi) {
     if (sys->d.dyn_box) {
-      if (obs) k_force<KIND, true, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force<KIND, true, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      if (obs) k_force<KIND, true, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, true, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
     } else {
-      if (obs) k_force<KIND, true, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force<KIND, true, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      if (obs) k_force<KIND, true, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, true, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
     }
   } else {
     if (sys->d.dyn_box) {
-      if (obs) k_force<KIND, false, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force<KIND, false, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      if (obs) k_force<KIND, false, true, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, false, false, FOLD, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
     } else {
-      if (obs) k_force<KIND, false, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
-      else k_force<KIND, false, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp);
+      if (obs) k_force<KIND, false, true, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, false, false, FOLD, false><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
     }
   }
 }
 
-int launch_force(md_system *sys, bool observables, double half_dt) {
+int launch_force(md_system *sys, bool observables, double half_dt, const StepCtl *ctlp) {
   const KickParams kp = make_kick(sys, half_dt);
+  cudaGraphConditionalHandle none{};
+  const StepCtl ctl = ctlp ? *ctlp : make_ctl(sys, 0.0, none, false, false);
   const int grid = force_blocks(sys);
   {
     ProfScope p(sys, MD_K_FORCE);
     if (sys->d.kind == MD_POT_TBSMA) {
-      if (sys->d.tb.fold) launch_force_k<MD_POT_TBSMA, true>(sys, grid, observables, kp);
-      else launch_force_k<MD_POT_TBSMA, false>(sys, grid, observables, kp);
-    } else launch_force_k<MD_POT_EAM_TABLE, true>(sys, grid, observables, kp);
+      if (sys->d.tb.fold) launch_force_k<MD_POT_TBSMA, true>(sys, grid, observables, kp, ctl);
+      else launch_force_k<MD_POT_TBSMA, false>(sys, grid, observables, kp, ctl);
+    } else launch_force_k<MD_POT_EAM_TABLE, true>(sys, grid, observables, kp, ctl);
   }
   if (observables) {
     ProfScope p(sys, MD_K_REDUCE);

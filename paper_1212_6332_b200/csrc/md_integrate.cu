@@ -9,34 +9,24 @@
 namespace md {
 
 
-// v += (dt/2m) f;  x += dt v;  d2 = |x - x_ref|^2  -> block max -> atomicMax on the bit pattern.
-__global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ DevSys s, const KickParams p, double dt) {
+// v += (dt/2m) f;  x += dt v;  d2 = |x - x_ref|^2  -> block max -> atomicMax on the bit pattern; the last block decides
+// whether the list is rebuilt (finish_displacement).  drift_atom is shared with the chained epilogue of the force pass
+// (md_force.cu), so that a step gives the same bits whichever kernel performs its drift.
+__global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ DevSys s, const KickParams p, const StepCtl ctl) {
+  __shared__ unsigned long long sm[8];
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const size_t N = (size_t)s.N;
   double d2 = 0.0;
   if (i < s.N) {
     double4 x = s.pos[i];
     double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
+    const double rx = s.xref[i], ry = s.xref[N + i], rz = s.xref[2 * N + i];
     half_kick(p, s.nt > 1 ? (int)x.w : 0, s.frc[i], s.frc[N + i], s.frc[2 * N + i], vx, vy, vz);
-    x.x += dt * vx; x.y += dt * vy; x.z += dt * vz;
+    d2 = drift_atom(ctl.dt, x, vx, vy, vz, rx, ry, rz);
     s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
     s.pos[i] = x;
-    const double ux = x.x - s.xref[i], uy = x.y - s.xref[N + i], uz = x.z - s.xref[2 * N + i];
-    d2 = ux * ux + uy * uy + uz * uz;
-    if (!(d2 == d2)) d2 = __longlong_as_double(0x7ff0000000000000ll);   // NaN -> +inf: forces a rebuild, which flags it
   }
-  // non-negative doubles order like their bit patterns
-  unsigned long long b = (unsigned long long)__double_as_longlong(d2);
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o); b = t > b ? t : b; }
-  __shared__ unsigned long long sm[8];
-  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = b;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-#pragma unroll
-    for (int w = 1; w < 8; ++w) b = sm[w] > b ? sm[w] : b;
-    if (b) atomicMax(&s.st->maxd2_bits, b);
-  }
+  finish_displacement(s, ctl, d2, sm);
 }
 
 KickParams make_kick(const md_system *sys, double half_dt) {
@@ -51,10 +41,10 @@ KickParams make_kick(const md_system *sys, double half_dt) {
   return k;
 }
 
-int launch_kick_drift(md_system *sys, double dt) {
+int launch_kick_drift(md_system *sys, double dt, const StepCtl &ctl) {
   ProfScope p(sys, MD_K_INTEGRATE);
   const KickParams kp = make_kick(sys, 0.5 * dt);
-  ++sys->launches, k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, kp, dt);
+  ++sys->launches, k_kick_drift<<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, kp, ctl);
   return (int)cudaGetLastError();
 }
 

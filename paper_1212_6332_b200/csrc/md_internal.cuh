@@ -22,8 +22,8 @@ constexpr double kAmuToEvFs2PerA2 = 103.642696526805;  // 1 amu (A/fs)^2 in eV
 
 // Device-resident mutable state (one per system).
 struct DevState {
-  unsigned long long maxd2_bits;   // bit pattern of max_i |x_i - x_ref,i|^2 since the last check (>=0 doubles order as u64)
-  double last_maxd2;               // value consumed by the last rebuild decision
+  unsigned long long maxd2_bits;   // bit pattern of max_i |x_i - x_ref,i|^2 since the last BUILD (>=0 doubles order as u64)
+  double last_maxd2;               // its value at the last rebuild decision
   int force_rebuild;               // host request: rebuild at the next decision point
   int do_rebuild;                  // decision of the current rebuild chain
   int error_flags;                 // MD_FLAG_* (sticky)
@@ -33,6 +33,7 @@ struct DevState {
   double box[3];                   // CURRENT box edges (md_create's, then scaled by the barostat): every kernel reads them here
   double mu, pressure;             // last barostat step
   unsigned long long graph_body_runs; // rebuild bodies that ran inside a CUDA-graph step (for the launch count)
+  unsigned long long step_word;    // running drift / chained force kernel: blocks arrived (low half) | blocks with an atom beyond skin/2 (high half)
 };
 
 struct TbsmaParams {               // per type pair, pre-combined on the host
@@ -95,12 +96,62 @@ struct DevSys {
   TableParams tab;
 };
 
+// What the kernel that ends a drift needs for the rebuild decision (taken by its last block, decide_rebuild below):
+// chain != 0 (force pass only): the epilogue also does the NEXT step's first half-kick, drift and displacement check.
+struct StepCtl { double dt; unsigned long long thr2_bits; cudaGraphConditionalHandle cond; int use_cond; int chain; };
+
 // first entry of the list row of the atom in (tile, lane); entry k is at row[(k >> 2) * 128 + (k & 3)]
 __host__ __device__ inline size_t nbr_row_offset(size_t tile, int cap, int lane) { return (tile * (size_t)(cap >> 2) * 32 + lane) * 4; }
 __host__ __device__ inline unsigned nbr_entry(int k) { return ((unsigned)k >> 2) * 128u + ((unsigned)k & 3u); }   // 32-bit: one IMAD.WIDE per store
 
 // current box edge a: a kernel parameter until a barostat is switched on, device state from then on
 __device__ __forceinline__ double box_edge(const DevSys &s, int a) { return s.dyn_box ? s.st->box[a] : s.L0[a]; }
+
+// The rebuild decision, on the device (one thread): rebuild if the host asked for it or if some atom has moved more
+// than skin/2 since the last build (`exceeded`: strict >, reading A11).  Inside a CUDA-graph step `cond` is the handle of
+// the conditional node whose body is the rebuild chain; otherwise every kernel of the chain is launched and returns at
+// once unless do_rebuild is set.
+__device__ __forceinline__ void decide_rebuild(const DevSys &s, bool exceeded, cudaGraphConditionalHandle cond, int use_cond) {
+  DevState *st = s.st;
+  const bool go = *(volatile int *)&st->force_rebuild != 0 || exceeded;
+  st->do_rebuild = go ? 1 : 0;
+  st->last_maxd2 = __longlong_as_double((long long)*(volatile unsigned long long *)&st->maxd2_bits);
+  st->force_rebuild = 0;
+  if (go) {
+    st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1;
+    for (int a = 0; a < 3; ++a)                        // the cell grid is fixed at md_create; a barostat may have shrunk the box
+      if (!(box_edge(s, a) >= s.nc[a] * s.rl)) st->error_flags |= MD_FLAG_BOX;
+  }
+  if (use_cond) { cudaGraphSetConditional(cond, go ? 1u : 0u); if (go) st->graph_body_runs += 1; }
+}
+
+// End of a drift (k_kick_drift, or the chained epilogue of the force pass): d2 = |x - x_ref|^2 of this thread's atom
+// (0 for a thread without one).  Thread 0 of every block adds ONE word to DevState::step_word: the low half counts the
+// blocks that have arrived, the high half those in which some atom exceeded skin/2.  The block that completes the count
+// reads the decision off the value the atomic returns, so no fence, no second round trip and no separate decision
+// kernel is needed; a block's resources are held for one L2 round trip after its last warp has finished.
+// maxd2_bits (bit pattern of the largest d2 since the last build: non-negative doubles order like their bit patterns)
+// is kept for md_stats and for md_set_positions; nothing waits for that reduction.
+// Called by every thread of the block; sm holds blockDim.x / 32 entries.
+__device__ __forceinline__ void finish_displacement(const DevSys &s, const StepCtl &c, double d2, unsigned long long *sm) {
+  if (!(d2 == d2)) d2 = __longlong_as_double(0x7ff0000000000000ll);   // NaN -> +inf: forces a rebuild, which flags it
+  unsigned long long b = (unsigned long long)__double_as_longlong(d2);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { const unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o); b = t > b ? t : b; }
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = b;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) b = sm[w] > b ? sm[w] : b;
+    DevState *st = s.st;
+    if (b) atomicMax(&st->maxd2_bits, b);
+    const unsigned long long inc = 1ull | (b > c.thr2_bits ? (1ull << 32) : 0ull);
+    const unsigned long long w = atomicAdd(&st->step_word, inc) + inc;
+    if ((unsigned)(w & 0xffffffffull) == gridDim.x) {
+      st->step_word = 0ull;                              // for the next kernel that ends a drift
+      decide_rebuild(s, (w >> 32) != 0ull, c.cond, c.use_cond);
+    }
+  }
+}
 
 struct ProfClass { std::vector<cudaEvent_t> ev; size_t used = 0; long dropped = 0; };
 
@@ -116,7 +167,8 @@ struct md_system {
   bool have_list, forces_valid, observables_valid;
   bool opt_step_obs, opt_profile, opt_graph;
   // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
-  cudaGraph_t step_graph; cudaGraphExec_t step_exec; double step_dt; bool step_obs; int step_kernels, body_kernels;
+  struct StepGraph { cudaGraph_t graph; cudaGraphExec_t exec; double dt; bool obs; int nsteps, kernels; } sg[2];   // [0]: kStepUnroll steps, [1]: the remainder
+  int body_kernels;
   int graph_error;                 // cudaError_t of a failed step-graph build (0: none); md_step then uses plain launches
   bool last_step_graph;            // the last md_step replayed the graph
   bool frc_keep;                   // frc holds the forces of the coordinates BEFORE the barostat scaled them: queries must not replace them
@@ -136,27 +188,38 @@ KickParams make_kick(const md_system *s, double half_dt);
 __device__ __forceinline__ void half_kick(const KickParams &k, int t, double fx, double fy, double fz, double &vx, double &vy, double &vz) {
   double g = 0.0;
   if (k.gdt != 0.0) {
-    const double v2 = (vx * vx + vy * vy) + vz * vz;
+    const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
     if (v2 > 0.0) g = k.gdt * (1.0 - k.c2[t] / v2);
   }
   const double h = k.h[t];
-  vx = vx + h * fx - g * vx; vy = vy + h * fy - g * vy; vz = vz + h * fz - g * vz;
+  // explicit FMAs: the same bits from every kernel that inlines this, whatever else it does with h, f or v
+  vx = fma(-g, vx, fma(h, fx, vx)); vy = fma(-g, vy, fma(h, fy, vy)); vz = fma(-g, vz, fma(h, fz, vz));
+}
+// x += dt v and the squared displacement from x_ref = (rx, ry, rz) (explicit FMAs: the same bits from every kernel that inlines this)
+__device__ __forceinline__ double drift_atom(double dt, double4 &x, double vx, double vy, double vz, double rx, double ry, double rz) {
+  x.x = fma(dt, vx, x.x); x.y = fma(dt, vy, x.y); x.z = fma(dt, vz, x.z);
+  const double ux = x.x - rx, uy = x.y - ry, uz = x.z - rz;
+  return fma(uz, uz, fma(uy, uy, ux * ux));
 }
 // launch geometry of the per-atom kernels that use the tile mapping
 constexpr int kForceBlock = 128;
 constexpr int kSubMaxAtoms = 24576;                // at or below this many atoms the passes use 8 lanes per atom (md_force.cu)
-bool use_sub_lanes(const md_system *s);
+constexpr int kSub32MaxAtoms = 4096;               // ... and 32 lanes per atom at or below this many
+constexpr int kSub32Limit = 32768;                 // largest system the 32-lane variant may be forced on (sizes the block partials)
+constexpr int kStepUnroll = 8;                     // time steps per CUDA graph of md_step (md_api.cu)
+int sub_lanes(const md_system *s);                 // lanes per atom of the two passes: 1, 2, 4, 8 or 32
 int force_blocks(const md_system *s);              // grid of the two passes (and number of block partials)
 inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block; }
 
 // launchers (each enqueues on s->stream; returns cudaError_t of the launch)
 int launch_rebuild_chain(md_system *s);                       // decision + body, conditional on DevState (force_rebuild / maxd2)
 int launch_decide(md_system *s, cudaGraphConditionalHandle cond, bool use_cond);
+StepCtl make_ctl(const md_system *s, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain);
 int launch_rebuild_body(md_system *s);
 int launch_density(md_system *s);
 int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
-int launch_force(md_system *s, bool observables, double half_dt); // half_dt = dt/2 (0: no velocity update)
-int launch_kick_drift(md_system *s, double dt);
+int launch_force(md_system *s, bool observables, double half_dt, const StepCtl *ctl = nullptr); // half_dt = dt/2 (0: no velocity update); ctl->chain: + next drift
+int launch_kick_drift(md_system *s, double dt, const StepCtl &ctl);
 int launch_ekin(md_system *s);
 int launch_barostat(md_system *s, double dt);                 // ekin, mu and box update, scale positions (end of a step)
 int launch_pressure(md_system *s);                            // ekin + eq.(6) into DevState::pressure

@@ -23,27 +23,15 @@ __device__ __forceinline__ int cell_coord(double x, double scale, int nc) {
 }
 
 // ---- K0: decision (one thread), then clear the cell counters -------------------------------------
-// The decision is taken on the device: rebuild if the host asked for it or if the largest displacement since the
-// last build exceeds skin/2 (strict >, reading A11).  When md_step runs as a CUDA graph, the rest of the chain sits
-// in the body of a conditional IF node and `cond` is its handle; otherwise every kernel of the chain is launched
-// and returns at once unless do_rebuild is set.
+// decide_rebuild (md_internal.cuh) as a kernel of its own: explicit builds and force evaluations outside md_step.
+// Inside md_step the last block of the kernel that ends a drift takes the decision (finish_displacement).
 __global__ void k_decide(const __grid_constant__ DevSys s, unsigned long long thr2_bits, cudaGraphConditionalHandle cond, int use_cond) {
-  DevState *st = s.st;
-  const bool go = st->force_rebuild != 0 || st->maxd2_bits > thr2_bits;
-  st->do_rebuild = go ? 1 : 0;
-  st->last_maxd2 = __longlong_as_double((long long)st->maxd2_bits);
-  st->maxd2_bits = 0ull;
-  st->force_rebuild = 0;
-  if (go) {
-    st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1;
-    for (int a = 0; a < 3; ++a)                        // the cell grid is fixed at md_create; a barostat may have shrunk the box
-      if (!(box_edge(s, a) >= s.nc[a] * s.rl)) st->error_flags |= MD_FLAG_BOX;
-  }
-  if (use_cond) { cudaGraphSetConditional(cond, go ? 1u : 0u); if (go) st->graph_body_runs += 1; }
+  decide_rebuild(s, s.st->maxd2_bits > thr2_bits, cond, use_cond);
 }
 
 __global__ void k_clear_cells(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
+  if (blockIdx.x == 0 && threadIdx.x == 0) s.st->maxd2_bits = 0ull;      // x_ref <- x below: the displacement starts from 0 again
   for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= s.ncell; c += gridDim.x * blockDim.x) { s.cell_count[c] = 0; s.cell_fill[c] = 0; }
 }
 
@@ -328,11 +316,17 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   }
 }
 
+StepCtl make_ctl(const md_system *sys, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain) {
+  StepCtl c;
+  c.dt = dt; c.thr2_bits = (unsigned long long)__builtin_bit_cast(long long, sys->d.thr2);
+  c.cond = cond; c.use_cond = use_cond ? 1 : 0; c.chain = chain ? 1 : 0;
+  return c;
+}
+
 int launch_decide(md_system *sys, cudaGraphConditionalHandle cond, bool use_cond) {
-  const DevSys &d = sys->d;
-  const unsigned long long thr_bits = (unsigned long long)__builtin_bit_cast(long long, d.thr2);
+  const StepCtl c = make_ctl(sys, 0.0, cond, use_cond, false);
   ProfScope p(sys, MD_K_BIN);
-  ++sys->launches, k_decide<<<1, 1, 0, sys->stream>>>(d, thr_bits, cond, use_cond ? 1 : 0);
+  ++sys->launches, k_decide<<<1, 1, 0, sys->stream>>>(sys->d, c.thr2_bits, cond, c.use_cond);
   return (int)cudaGetLastError();
 }
 

@@ -165,11 +165,12 @@ def test_step_with_observables_matches_plain_step(md):
     assert np.abs(a.positions() - b.positions()).max() < 1e-11 and np.abs(a.velocities() - b.velocities()).max() < 1e-12
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 @pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3b_small", "cfg4_small", "alloy_tbsma",
                                   "alloy_tables", "alloy_tbsma_rcut", "alloy_tables_rcut"] + NEW_VARIANT_CASES)
 def test_both_pass_variants(md, case, variant):
-    """One thread per atom (what large systems run) and 8 lanes per atom (small systems), forced on the same input."""
+    """One thread per atom (what large systems run), 8 / 32 lanes per atom (small systems) and 4 lanes per atom (long
+    rows), forced on the same input."""
     w = CASES[case]()
     o = oracle_of(w)
     of, oe, ow = o.compute_forces()
@@ -207,6 +208,26 @@ def test_graph_step_equals_plain_launches(md, case):
     a.step(5, 0.5 * w.dt)
     b.step(5, 0.5 * w.dt)
     assert np.array_equal(a.positions(), b.positions())
+
+
+@pytest.mark.parametrize("case", ["cfg0", "cfg2_small", "cfg4_small", "alloy_tables_rcut"])
+@pytest.mark.parametrize("graph", [1, 0])
+def test_chained_steps_equal_single_steps(md, case, graph):
+    """md_step(n) chains the steps (the force pass of a step performs the next step's first half-kick, drift and
+    displacement check; several steps per CUDA graph); n calls of md_step(1) do not.  Same bits either way."""
+    w = CASES[case]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    for s in (a, b):
+        s.set_option(md.MD_OPT_GRAPH, graph)
+    a.step(43, w.dt)                                  # 5 graphs of 8 steps + one of 3
+    for _ in range(43):
+        b.step(1, w.dt)
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    sa, sb = a.stats(), b.stats()
+    assert sa["rebuilds"] == sb["rebuilds"] and sa["rebuilds"] >= 2 and sa["error_flags"] == 0
+    assert sa["kernel_launches"] < sb["kernel_launches"] and sa["graph_active"] == graph
+    fa, fb = a.compute_forces()[0], b.compute_forces()[0]
+    assert np.array_equal(fa, fb)
 
 
 @pytest.mark.parametrize("case,variant", [("cfg0", 0), ("alloy_tbsma", 1), ("alloy_tables", 2), ("cfg2_small", 0)])
