@@ -260,6 +260,10 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
     g = md.MDSystem(w)
     if args.no_graph:
         g.set_option(md.MD_OPT_GRAPH, 0)
+    if args.variant:
+        g.set_option(md.MD_OPT_FORCE_VARIANT, args.variant)
+    if args.half is not None:
+        g.set_option(md.MD_OPT_HALF_LIST, args.half)
     stream = torch.cuda.current_stream()
 
     # ---- device-resident run: W warm-up steps, then exactly K timed steps ------------------------------
@@ -368,7 +372,7 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "n_atoms_per_gpu": w.n_atoms, "n_boxes": w.n_boxes, "cutoff": w.cutoff, "skin": w.skin,
                        "dt_fs": w.dt, "parallelism": "replicas only (one independent system per GPU, no collective)",
-                       "rebuilds_in_timed_region": rebuilds, "mean_list_entries": st2["list_entries"] / w.n_atoms,
+                       "rebuilds_in_timed_region": rebuilds, "force_variant": args.variant, "half_list": args.half, "mean_list_entries": st2["list_entries"] / w.n_atoms,
                        "l2": f"no flush: per-step working set (neighbour list {4 * st2['list_entries'] / 2 ** 20:.0f} MiB + per-atom "
                              f"arrays, workspace {ws_mb:.0f} MiB) exceeds the 126 MB L2" if 4 * st2["list_entries"] > 126e6
                              else "no flush: working set fits L2 (small config; steady-state MD keeps it there by design)"},
@@ -392,6 +396,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="cap on the end-to-end steps (0: same as --steps)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", type=int, default=0, help="MD_OPT_FORCE_VARIANT (lanes per atom; 0: chosen by system size)")
+    ap.add_argument("--half", type=int, default=None,
+                    help="MD_OPT_HALF_LIST (bit 0: density pass, bit 1: force pass use Newton's third law; default: the library's choice)")
     ap.add_argument("--no-graph", action="store_true",
                     help="plain kernel launches instead of one CUDA graph per step (for ncu launch lists: ncu does not list "
                          "kernels launched from a graph with a conditional node)")

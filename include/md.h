@@ -184,8 +184,17 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                           the next step's first half-kick, drift and displacement check, and the last block of that
  *                           kernel takes the rebuild decision (2 kernel launches per step when no rebuild is due);
  *                           0: the same kernels as plain launches (every kernel of the rebuild chain is launched and
- *                           returns at once unless a rebuild is due).  MD_OPT_PROFILE implies plain launches. */
-enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3, MD_OPT_GRAPH = 4 };
+ *                           returns at once unless a rebuild is due).  MD_OPT_PROFILE implies plain launches.
+ *  MD_OPT_HALF_LIST         Newton's third law (the paper's CPU code uses it, its GPU kernels do not).  Bit 0:
+ *                           the density pass, bit 1: the force pass evaluates every undirected pair ONCE, on the atom
+ *                           that owns it, and sends the partner's share by 64-bit integer reductions in units of
+ *                           2^-43 (deterministic: integer sums do not depend on the order of arrival; each received
+ *                           contribution is rounded to 1.1e-13 eV/A, eV or density units, sums must stay below 1e6).  Takes effect for systems
+ *                           that run one thread per atom with a static box (every row of the list holds the pairs
+ *                           its atom owns first, so no rebuild is needed).  -1 (default): the library's choice from
+ *                           its measurements on B200: 1 for MD_POT_EAM_TABLE (the table passes are bound by the
+ *                           gathers, not by arithmetic), 0 for MD_POT_TBSMA (full lists, as the paper's GPU kernels). */
+enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3, MD_OPT_GRAPH = 4, MD_OPT_HALF_LIST = 5 };
 int md_set_option(md_system *s, int option, int value);
 
 /* Kernel classes for md_profile_read */

@@ -114,6 +114,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   t.scan_block = b.take<int>(4096);
   t.nbr = b.take<unsigned>((size_t)d->n_boxes * g.tiles_per_box * g.cap * 32);
   t.ncount = b.take<int>(N);
+  t.nown = b.take<int>(N); t.rho_fix = b.take<long long>(N); t.frc_fix = b.take<long long>(4 * N);
   t.rho = b.take<double>(N); t.eemb = b.take<double>(N); t.eatom = b.take<double>(N);
   t.partial = b.take<double>((size_t)g.n_blocks * 8);
   t.box_epot = b.take<double>(d->n_boxes); t.box_virial = b.take<double>((size_t)d->n_boxes * 6);
@@ -134,6 +135,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
     o.frc = t.frc; o.xref = t.xref; o.type = t.type; o.type_tmp = t.type_tmp; o.orig = t.orig; o.orig_tmp = t.orig_tmp;
     o.cell_id = t.cell_id; o.perm = t.perm; o.cell_count = t.cell_count; o.cell_start = t.cell_start;
     o.cell_fill = t.cell_fill; o.scan_block = t.scan_block; o.nbr = t.nbr; o.ncount = t.ncount; o.rho = t.rho;
+    o.nown = t.nown; o.rho_fix = t.rho_fix; o.frc_fix = t.frc_fix;
     o.eemb = t.eemb; o.eatom = t.eatom; o.partial = t.partial; o.box_epot = t.box_epot; o.box_virial = t.box_virial;
     o.box_ekin = t.box_ekin;
     o.tab.f_val = tabs[0]; o.tab.f_der = tabs[1]; o.tab.phi_val = tabs[2]; o.tab.phi_der = tabs[3];
@@ -408,6 +410,16 @@ static int build_step_graph(md_system *s, md_system::StepGraph &sg, double dt, b
   return MD_OK;
 }
 
+// The passes that run as half passes depend on three settings (MD_OPT_HALF_LIST, the lanes per atom, the barostat);
+// every row holds its owned pairs first whatever the setting, so a change only invalidates the forces.
+static void refresh_half(md_system *s) {
+  const int h = half_mask(s);
+  if (h == s->d.half) return;
+  s->d.half = h;
+  drop_step_graph(s);
+  s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;
+}
+
 static int request_rebuild(md_system *s) {
   const int one = 1;
   return check_cuda(cudaMemcpyAsync(&s->d.st->force_rebuild, &one, sizeof(int), cudaMemcpyHostToDevice, s->stream));
@@ -467,7 +479,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->stream = (cudaStream_t)d->stream;
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
-  s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->steps = 0; s->launches = 0;
+  s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->opt_half = -1; s->steps = 0; s->launches = 0;
   s->thermo_Te = 0.0; s->thermo_tau = 0.0; s->baro_P0 = 0.0; s->baro_tau = 0.0;
   for (auto &g : s->sg) { g.graph = nullptr; g.exec = nullptr; g.dt = 0.0; g.obs = false; g.nsteps = 0; g.kernels = 0; }
   s->body_kernels = 0;
@@ -558,9 +570,12 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
     if (e == cudaSuccess) { ++s->launches, k_set_vec<<<grid_for(o.N), 256, 0, st>>>(o, o.vel, vdev); e = cudaGetLastError(); }
   }
   if (e == cudaSuccess) e = cudaMemsetAsync(o.frc, 0, 3 * N * sizeof(double), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(o.rho_fix, 0, N * sizeof(long long), st);      // the half passes leave them zero
+  if (e == cudaSuccess) e = cudaMemsetAsync(o.frc_fix, 0, 4 * N * sizeof(long long), st);
   int flags = 0;
   if (e != cudaSuccess || sync_and_flags(s, &flags) == MD_ECUDA) { delete s; cudaGetLastError(); return MD_ECUDA; }
   if (flags & (1 << 30)) { delete s; return MD_EINVAL; }   // a type out of range
+  s->d.half = half_mask(s);
   *out = s;
   return MD_OK;
 }
@@ -582,7 +597,10 @@ int md_set_option(md_system *s, int option, int value) {
     case MD_OPT_GRAPH: s->opt_graph = value != 0; if (value) s->graph_error = 0; return MD_OK;   // switching it on retries a failed build
     case MD_OPT_FORCE_VARIANT:
       if (value < 0 || value > 4 || (value == 3 && s->d.N > kSub32Limit)) return MD_EINVAL;
-      s->opt_force_variant = value; drop_step_graph(s); return MD_OK;
+      s->opt_force_variant = value; drop_step_graph(s); refresh_half(s); return MD_OK;
+    case MD_OPT_HALF_LIST:
+      if (value < -1 || value > 3) return MD_EINVAL;
+      s->opt_half = value; refresh_half(s); return MD_OK;
   }
   return MD_EINVAL;
 }
@@ -604,6 +622,7 @@ int md_set_barostat(md_system *s, double P0, double tau_p) {
         cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
     s->d.dyn_box = 0;
   }
+  refresh_half(s);
   return MD_OK;
 }
 

@@ -310,6 +310,18 @@ __device__ __forceinline__ const double4 *slot_ptr(const double4 *base, unsigned
   return (const double4 *)a;
 }
 
+// Half passes (MD_OPT_HALF_LIST): the partner's share of a pair term, as a 64-bit integer reduction in units of 2^-43.
+// The result of the atomic is not used, so it is a fire-and-forget RED.E.ADD.64; integer sums are order-independent.
+__device__ __forceinline__ void red_fix(long long *p, double v) {
+  const long long q = __double2ll_rn(v * kFixScale);
+  if (q) atomicAdd(reinterpret_cast<unsigned long long *>(p), (unsigned long long)q);
+}
+__device__ __forceinline__ double fix_take(long long *p) {        // read a received sum and clear it for the next pass
+  const long long q = *p;
+  if (q) *p = 0;
+  return (double)q * kFixInv;
+}
+
 // eval2 evaluates two pairs at once: their dependency chains are independent (measured on B200: one dependent DFMA
 // chain per warp tops out at 64 % of the FP64 pipe, two at 77 %, four at 90 %).
 template <class Prep, class Eval2, class Eval1>
@@ -431,7 +443,7 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
   }
 }
 
-template <int KIND, bool MULTI, bool FOLD, bool DYN>
+template <int KIND, bool MULTI, bool FOLD, bool DYN, bool HALF = false>
 __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s) {
   __shared__ double tab_sm[kExpTabLen];
   // the atom's own loads are issued BEFORE the table staging and its barrier, so that their latency overlaps it
@@ -446,6 +458,9 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int ti = MULTI ? (int)pi.w : 0;
   double rho = 0.0, rho2 = 0.0;
+  // HALF: only the pairs this atom owns (they come first in the row); the partner gets its share by red_fix
+  const int own = HALF && valid ? s.nown[i] : 0;
+  const int n_main = HALF ? (own & 0xffff) : row.n_in, n_tail = HALF ? (own >> 16) : row.n_out;
 
   // main part: branch-free.  TB-SMA: the clamped switch makes a pair beyond r_c contribute exactly 0;
   // tables (no switch, reading A9): the strict test r2 < rc2 selects the term.
@@ -456,16 +471,19 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
     return d;
   };
   auto term1 = [&](const PairD &d) {
-    const double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)d.w : 0, d.r2);
-    return (KIND == MD_POT_TBSMA || d.r2 < (MULTI ? s.rc2p[ti * s.nt + (int)d.w] : s.rc2)) ? term : 0.0;
+    double term = density_term<KIND, MULTI, FOLD>(s, lc, tab, MULTI ? ti * s.nt + (int)d.w : 0, d.r2);
+    term = (KIND == MD_POT_TBSMA || d.r2 < (MULTI ? s.rc2p[ti * s.nt + (int)d.w] : s.rc2)) ? term : 0.0;
+    if (HALF) red_fix(s.rho_fix + MD_GIDX(d.e), term);              // rho^(ab) is symmetric in (a, b)
+    return term;
   };
-  walk_main(row.main, row.n_in, s.pos, prep,
+  walk_main(row.main, n_main, s.pos, prep,
             [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
                 const double r2v[2] = {a.r2, b.r2};
                 double tv[2];
                 density_term_n<FOLD, 2>(s, lc, tab, r2v, tv);
                 rho += tv[0]; rho2 += tv[1];
+                if (HALF) { red_fix(s.rho_fix + MD_GIDX(a.e), tv[0]); red_fix(s.rho_fix + MD_GIDX(b.e), tv[1]); }
               } else {
                 rho += term1(a); rho2 += term1(b);
               }
@@ -475,12 +493,12 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
 
   // skin part: distance test only; a pair found inside r_c is parked (one slot per lane) and the warp evaluates
   // the parked pairs together when some lane needs its slot again, and once at the end
-  const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
+  const int mg = (__reduce_max_sync(0xffffffffu, n_tail) + 3) >> 2;
   // only the ENTRY is parked (one register); the rare evaluation gathers and prepares the pair again
   unsigned park = 0u;
   bool parked = false;
   auto flush = [&]() { rho += term1(prep(park, gather32(slot_ptr(s.pos, MD_GIDX(park))))); parked = false; };
-  walk_tail(row.last, row.n_out, mg, s.pos, prep, [&](const PairD &d, bool active) {
+  walk_tail(row.last, n_tail, mg, s.pos, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
       if (parked) flush();
@@ -492,9 +510,25 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   }
 
   if (!valid) return;
+  if (HALF) { s.rho[i] = rho; return; }                            // the owned part; k_embed adds what the partners sent
   double F, Fp;
   embed<KIND>(s, ti, rho, F, Fp);
   if (!(fabs(Fp) <= 1.79e308) || !(fabs(rho) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);   // r = 0 or overflow
+  s.rho[i] = rho;
+  s.eemb[i] = F;
+  s.posf[i] = make_double4(pi.x, pi.y, pi.z, Fp);
+}
+
+// Second kernel of a half density pass: rho_i = owned part + received part; F(rho_i), F'(rho_i)
+template <int KIND>
+__global__ void __launch_bounds__(256) k_embed(const __grid_constant__ DevSys s) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const double4 pi = s.pos[i];
+  const double rho = s.rho[i] + fix_take(s.rho_fix + i);
+  double F, Fp;
+  embed<KIND>(s, s.nt > 1 ? (int)pi.w : 0, rho, F, Fp);
+  if (!(fabs(Fp) <= 1.79e308) || !(fabs(rho) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
   s.rho[i] = rho;
   s.eemb[i] = F;
   s.posf[i] = make_double4(pi.x, pi.y, pi.z, Fp);
@@ -581,65 +615,96 @@ __device__ __forceinline__ void force_merge(ForceAcc<OBS> &a, const ForceAcc<OBS
   if constexpr (OBS) { a.ev += b.ev; a.w0 += b.w0; a.w1 += b.w1; a.w2 += b.w2; a.w3 += b.w3; a.w4 += b.w4; a.w5 += b.w5; }
 }
 
-// Epilogue of the force pass for the thread that holds the totals of atom i (valid) or nothing (!valid): store the
-// force, second half-kick, non-finite flag; OBS: per-atom energy and the block's partial sums of E and W.
-// ctl.chain: the same thread goes on with the NEXT step's first half-kick and drift (the new position goes to `pos`,
-// which this pass does not read: it gathers from `posf`) and the displacement check, so that a step inside md_step
-// costs two kernels (density, force) instead of four.
+// Epilogue of the force pass, in three pieces (a half pass runs them in two kernels).
+// (1) the atom: store the force, second half-kick, non-finite flag.  ctl.chain: the same thread goes on with the NEXT
+// step's first half-kick and drift (the new position goes to `pos`, which this pass does not read: it gathers from
+// `posf`), so that a step inside md_step costs two kernels (density, force) instead of four.
+// Returns the squared displacement from x_ref after that drift (0 otherwise).
+__device__ __forceinline__ double atom_update(const DevSys &s, const KickParams &kick, const StepCtl &ctl, int i, int ti, const double4 &pi,
+                                              double fx, double fy, double fz) {
+  const size_t N = (size_t)s.N;
+  double d2 = 0.0;
+  if (kick.h[ti] != 0.0) {
+    // every load of the epilogue is issued before anything waits for one of them
+    double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
+    double rx = 0.0, ry = 0.0, rz = 0.0;
+    if (ctl.chain) { rx = s.xref[i]; ry = s.xref[N + i]; rz = s.xref[2 * N + i]; }
+    s.frc[i] = fx; s.frc[N + i] = fy; s.frc[2 * N + i] = fz;
+    half_kick(kick, ti, fx, fy, fz, vx, vy, vz);
+    if (ctl.chain) {
+      half_kick(kick, ti, fx, fy, fz, vx, vy, vz);
+      double4 x = make_double4(pi.x, pi.y, pi.z, (double)ti);
+      d2 = drift_atom(ctl.dt, x, vx, vy, vz, rx, ry, rz);
+      s.pos[i] = x;
+    }
+    s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
+  } else {
+    s.frc[i] = fx; s.frc[N + i] = fy; s.frc[2 * N + i] = fz;
+  }
+  if (!(fabs(fx) + fabs(fy) + fabs(fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
+  return d2;
+}
+
+// (2) observables: components [C0, C1) of this block's partial sums (0: energy, 1..6: virial), by warp shuffles in a
+// fixed butterfly order and then across the 4 warps (deterministic).  Called by every thread of the block.
+template <int C0, int C1>
+__device__ __forceinline__ void block_partials(const DevSys &s, double (&v)[7], double (*sm)[8]) {
+#pragma unroll
+  for (int c = C0; c < C1; ++c)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0)
+#pragma unroll
+    for (int c = C0; c < C1; ++c) sm[wid][c] = v[c];
+  __syncthreads();
+  if ((int)threadIdx.x >= C0 && (int)threadIdx.x < C1) {
+    double a = 0.0;
+#pragma unroll
+    for (int w = 0; w < kForceBlock / 32; ++w) a += sm[w][threadIdx.x];
+    s.partial[(size_t)blockIdx.x * 8 + threadIdx.x] = a;
+  }
+}
+
+// (1) + (2) + (3: the displacement check of a chained step) for the thread that holds the totals of atom i (valid) or
+// nothing (!valid)
 template <bool OBS>
 __device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &kick, const StepCtl &ctl, int i, bool valid, int ti,
                                              const double4 &pi, const ForceAcc<OBS> &acc, double (*sm)[8], unsigned long long *smd) {
-  double d2 = 0.0;
-  if (valid) {
-    const size_t N = (size_t)s.N;
-    if (kick.h[ti] != 0.0) {
-      // every load of the epilogue is issued before anything waits for one of them
-      double vx = s.vel[i], vy = s.vel[N + i], vz = s.vel[2 * N + i];
-      double rx = 0.0, ry = 0.0, rz = 0.0;
-      if (ctl.chain) { rx = s.xref[i]; ry = s.xref[N + i]; rz = s.xref[2 * N + i]; }
-      s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
-      half_kick(kick, ti, acc.fx, acc.fy, acc.fz, vx, vy, vz);
-      if (ctl.chain) {
-        half_kick(kick, ti, acc.fx, acc.fy, acc.fz, vx, vy, vz);
-        double4 x = make_double4(pi.x, pi.y, pi.z, (double)ti);
-        d2 = drift_atom(ctl.dt, x, vx, vy, vz, rx, ry, rz);
-        s.pos[i] = x;
-      }
-      s.vel[i] = vx; s.vel[N + i] = vy; s.vel[2 * N + i] = vz;
-    } else {
-      s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
-    }
-    if (!(fabs(acc.fx) + fabs(acc.fy) + fabs(acc.fz) <= 1.79e308)) atomicOr(&s.st->error_flags, MD_FLAG_NONFINITE);
-  }
+  const double d2 = valid ? atom_update(s, kick, ctl, i, ti, pi, acc.fx, acc.fy, acc.fz) : 0.0;
   if constexpr (OBS) {
     double e_i = 0.0;
     if (valid) { e_i = s.eemb[i] + 0.5 * acc.ev; s.eatom[i] = e_i; }
-    // warp-shuffle reduction (fixed butterfly order => deterministic), then across the 4 warps
     double v[7] = {e_i, 0.5 * acc.w0, 0.5 * acc.w1, 0.5 * acc.w2, 0.5 * acc.w3, 0.5 * acc.w4, 0.5 * acc.w5};
     if (!valid) {
 #pragma unroll
       for (int c = 0; c < 7; ++c) v[c] = 0.0;
     }
-#pragma unroll
-    for (int c = 0; c < 7; ++c)
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (lane == 0)
-#pragma unroll
-      for (int c = 0; c < 7; ++c) sm[wid][c] = v[c];
-    __syncthreads();
-    if (threadIdx.x < 7) {
-      double a = 0.0;
-#pragma unroll
-      for (int w = 0; w < kForceBlock / 32; ++w) a += sm[w][threadIdx.x];
-      s.partial[(size_t)blockIdx.x * 8 + threadIdx.x] = a;
-    }
+    block_partials<0, 7>(s, v, sm);
   }
   if (ctl.chain) finish_displacement(s, ctl, d2, smd);
 }
 
-template <int KIND, bool MULTI, bool OBS, bool FOLD, bool DYN>
+// Half pass, first kernel: the owned part of the force (and of sum V) goes to frc / eatom as it is, the virial partials
+// are complete (every undirected pair was evaluated exactly once: weight 1 where the full pass has 1/2 twice)
+template <bool OBS>
+__device__ __forceinline__ void force_park_half(const DevSys &s, int i, bool valid, const ForceAcc<OBS> &acc, double (*sm)[8]) {
+  if (valid) {
+    const size_t N = (size_t)s.N;
+    s.frc[i] = acc.fx; s.frc[N + i] = acc.fy; s.frc[2 * N + i] = acc.fz;
+  }
+  if constexpr (OBS) {
+    if (valid) s.eatom[i] = acc.ev;
+    double v[7] = {0.0, acc.w0, acc.w1, acc.w2, acc.w3, acc.w4, acc.w5};
+    if (!valid) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) v[c] = 0.0;
+    }
+    block_partials<1, 7>(s, v, sm);
+  }
+}
+
+template <int KIND, bool MULTI, bool OBS, bool FOLD, bool DYN, bool HALF = false>
 __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __grid_constant__ DevSys s, const KickParams kick, const StepCtl ctl) {
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
@@ -655,6 +720,15 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
   const int ti = MULTI ? s.type[i] : 0;
   ForceAcc<OBS> acc, acc2;
+  // HALF: only the pairs this atom owns (first in the row); the partner's share (-g d, and V) goes out by red_fix
+  const int own = HALF && valid ? s.nown[i] : 0;
+  const int n_main = HALF ? (own & 0xffff) : row.n_in, n_tail = HALF ? (own >> 16) : row.n_out;
+  auto send = [&](const PairD &d, double g, double V) {
+    const size_t N = (size_t)s.N;
+    long long *f = s.frc_fix + MD_GIDX(d.e);
+    red_fix(f, -g * d.dx); red_fix(f + N, -g * d.dy); red_fix(f + 2 * N, -g * d.dz);
+    if (OBS) red_fix(f + 3 * N, V);
+  };
 
   auto prep = [&](unsigned e, const double4 &pj) {
     PairD d;
@@ -668,8 +742,9 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     force_term<KIND, MULTI, OBS, FOLD>(s, lc, tab, tp, d.r2, pi.w + d.w, g, V);
     if (KIND != MD_POT_TBSMA && !(d.r2 < (MULTI ? s.rc2p[tp] : s.rc2))) { g = 0.0; V = 0.0; }   // tables: strict cut-off (A9)
     force_accumulate<OBS>(to, g, V, d.dx, d.dy, d.dz);
+    if (HALF) send(d, g, V);
   };
-  walk_main(row.main, row.n_in, s.posf, prep,
+  walk_main(row.main, n_main, s.posf, prep,
             [&](const PairD &a, const PairD &b) {
               if constexpr (KIND == MD_POT_TBSMA && !MULTI) {
                 const double r2v[2] = {a.r2, b.r2}, fpv[2] = {pi.w + a.w, pi.w + b.w};
@@ -677,6 +752,7 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
                 force_term_n<OBS, FOLD, 2>(s, lc, tab, r2v, fpv, gv, Vv);
                 force_accumulate<OBS>(acc, gv[0], Vv[0], a.dx, a.dy, a.dz);
                 force_accumulate<OBS>(acc2, gv[1], Vv[1], b.dx, b.dy, b.dz);
+                if (HALF) { send(a, gv[0], Vv[0]); send(b, gv[1], Vv[1]); }
               } else {
                 eval1(a, acc); eval1(b, acc2);
               }
@@ -685,11 +761,11 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   force_merge<OBS>(acc, acc2);
 
   // skin part: distance test only; pairs found inside r_c are parked and evaluated together (see k_density)
-  const int mg = (__reduce_max_sync(0xffffffffu, row.n_out) + 3) >> 2;
+  const int mg = (__reduce_max_sync(0xffffffffu, n_tail) + 3) >> 2;
   unsigned park = 0u;
   bool parked = false;
   auto flush = [&]() { eval1(prep(park, gather32(slot_ptr(s.posf, MD_GIDX(park)))), acc); parked = false; };
-  walk_tail(row.last, row.n_out, mg, s.posf, prep, [&](const PairD &d, bool active) {
+  walk_tail(row.last, n_tail, mg, s.posf, prep, [&](const PairD &d, bool active) {
     const bool hit = active && d.r2 < s.rc2;
     if (__any_sync(0xffffffffu, hit && parked)) {
       if (parked) flush();
@@ -700,8 +776,38 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
     if (parked) flush();
   }
 
-  force_finish<OBS>(s, kick, ctl, i, valid, ti, pi, acc, sm, smd);
+  if constexpr (HALF) force_park_half<OBS>(s, i, valid, acc, sm);
+  else force_finish<OBS>(s, kick, ctl, i, valid, ti, pi, acc, sm, smd);
 }
+
+// Half pass, second kernel (same block-to-atom mapping as k_force): total force = owned part + what the partners sent,
+// then the epilogue of the full pass (E_i = F(rho_i) + 1/2 (owned + received sum of V); its block partial is component 0)
+template <bool OBS>
+__global__ void __launch_bounds__(kForceBlock) k_force_half_finish(const __grid_constant__ DevSys s, const KickParams kick, const StepCtl ctl) {
+  __shared__ double sm[kForceBlock / 32][8];
+  __shared__ unsigned long long smd[kForceBlock / 32];
+  const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
+  const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
+  const bool valid = local < s.npb;
+  const int i = box * s.npb + (valid ? local : 0);
+  const size_t N = (size_t)s.N;
+  double d2 = 0.0, e_i = 0.0;
+  if (valid) {
+    const double4 pi = s.posf[i];
+    const int ti = s.nt > 1 ? s.type[i] : 0;
+    long long *f = s.frc_fix + i;
+    const double fx = s.frc[i] + fix_take(f), fy = s.frc[N + i] + fix_take(f + N), fz = s.frc[2 * N + i] + fix_take(f + 2 * N);
+    d2 = atom_update(s, kick, ctl, i, ti, pi, fx, fy, fz);
+    if (OBS) { e_i = s.eemb[i] + 0.5 * (s.eatom[i] + fix_take(f + 3 * N)); s.eatom[i] = e_i; }
+  }
+  if constexpr (OBS) {
+    double v[7] = {e_i, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    block_partials<0, 1>(s, v, sm);
+  }
+  if (ctl.chain) finish_displacement(s, ctl, d2, smd);
+}
+
+
 
 // ------------------------------------------------------------------------------------------------
 // Small systems: kSub lanes per atom.  With one thread per atom a system of a few thousand atoms fills a fraction of
@@ -889,6 +995,15 @@ int sub_lanes(const md_system *sys) {
   if (sys->d.N <= kSub32MaxAtoms) return 32;
   return sys->d.N <= kSubMaxAtoms ? 8 : 1;
 }
+// passes that run as half passes (MD_OPT_HALF_LIST): only with one thread per atom and a static box
+// opt_half < 0 (default): chosen by what was measured on B200: the table passes are bound by the
+// L1 data pipe (two gathered sectors per pair in the density pass), where one reduction per pair is cheaper than the
+// second evaluation; the TB-SMA passes are bound by FP64 issue and the force pass sends three reductions per pair: full.
+int half_mask(const md_system *sys) {
+  if (sub_lanes(sys) != 1 || sys->d.dyn_box) return 0;
+  if (sys->opt_half >= 0) return sys->opt_half;
+  return sys->d.kind == MD_POT_EAM_TABLE ? 1 : 0;
+}
 int force_blocks(const md_system *sys) {
   return sys->d.nb * blocks_per_box(sys->d.npb, kForceBlock / sub_lanes(sys));
 }
@@ -906,6 +1021,12 @@ static void launch_density_k(md_system *sys, int grid) {
     case 32: launch_density_sub<KIND, FOLD, 32>(sys, grid); return;
     case 8: launch_density_sub<KIND, FOLD, 8>(sys, grid); return;
     case 4: launch_density_sub<KIND, FOLD, 4>(sys, grid); return;
+  }
+  if (sys->d.half & 1) {
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    else k_density<KIND, false, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    ++sys->launches, k_embed<KIND><<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d);
+    return;
   }
   if (sys->d.dyn_box) {
     if (sys->d.nt > 1) k_density<KIND, true, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
@@ -947,6 +1068,19 @@ static void launch_force_k(md_system *sys, int grid, bool obs, const KickParams 
     case 32: launch_force_sub<KIND, FOLD, 32>(sys, grid, obs, kp, ctl); return;
     case 8: launch_force_sub<KIND, FOLD, 8>(sys, grid, obs, kp, ctl); return;
     case 4: launch_force_sub<KIND, FOLD, 4>(sys, grid, obs, kp, ctl); return;
+  }
+  if (sys->d.half & 2) {
+    if (multi) {
+      if (obs) k_force<KIND, true, true, FOLD, false, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, true, false, FOLD, false, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    } else {
+      if (obs) k_force<KIND, false, true, FOLD, false, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+      else k_force<KIND, false, false, FOLD, false, true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    }
+    ++sys->launches;
+    if (obs) k_force_half_finish<true><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    else k_force_half_finish<false><<<grid, kForceBlock, 0, st>>>(sys->d, kp, ctl);
+    return;
   }
   if (multi) {
     if (sys->d.dyn_box) {

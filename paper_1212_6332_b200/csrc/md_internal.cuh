@@ -86,6 +86,14 @@ struct DevSys {
   // Entries that were inside r_c at build time are at k = 0 .. n_in-1, the others at k = cap-n_out .. cap-1;
   // the unused entries of a partly filled group are 0; ncount = n_in | n_out << 16
   unsigned *nbr; int *ncount;
+  // Newton's-third-law variant (MD_OPT_HALF_LIST, row f2): `half` bit 0: density pass, bit 1: force pass.  The list build
+  // scans the half of the stencil whose pairs the atom OWNS first, so both parts of a row start with the owned pairs:
+  // nown = n_own_in | n_own_out << 16.  A half pass evaluates only those and sends the partner's share to rho_fix /
+  // frc_fix by 64-bit integer reductions in units of 2^-43 (integer addition is associative: the sums do not depend
+  // on the order of arrival)
+  int half; int *nown;
+  long long *rho_fix;              // [N]
+  long long *frc_fix;              // [4][N]: fx, fy, fz, sum of V (observables)
   const double *exp_tab;           // [kExpTabLen] 2^(j/64), correctly rounded (staged into shared memory by the passes), then LoopConsts
   // per-atom results
   double *rho, *eemb, *eatom;
@@ -99,6 +107,8 @@ struct DevSys {
 // What the kernel that ends a drift needs for the rebuild decision (taken by its last block, decide_rebuild below):
 // chain != 0 (force pass only): the epilogue also does the NEXT step's first half-kick, drift and displacement check.
 struct StepCtl { double dt; unsigned long long thr2_bits; cudaGraphConditionalHandle cond; int use_cond; int chain; };
+
+constexpr double kFixScale = 8796093022208.0, kFixInv = 1.0 / 8796093022208.0;   // 2^43: one unit = 1.1e-13 (eV/A, eV, density), range +-1.0e6
 
 // first entry of the list row of the atom in (tile, lane); entry k is at row[(k >> 2) * 128 + (k & 3)]
 __host__ __device__ inline size_t nbr_row_offset(size_t tile, int cap, int lane) { return (tile * (size_t)(cap >> 2) * 32 + lane) * 4; }
@@ -172,7 +182,7 @@ struct md_system {
   int graph_error;                 // cudaError_t of a failed step-graph build (0: none); md_step then uses plain launches
   bool last_step_graph;            // the last md_step replayed the graph
   bool frc_keep;                   // frc holds the forces of the coordinates BEFORE the barostat scaled them: queries must not replace them
-  int opt_force_variant;
+  int opt_force_variant, opt_half;
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
@@ -217,6 +227,7 @@ int launch_decide(md_system *s, cudaGraphConditionalHandle cond, bool use_cond);
 StepCtl make_ctl(const md_system *s, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain);
 int launch_rebuild_body(md_system *s);
 int launch_density(md_system *s);
+int half_mask(const md_system *s);                            // passes that run as half passes now (0 unless one thread per atom, static box)
 int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
 int launch_force(md_system *s, bool observables, double half_dt, const StepCtl *ctl = nullptr); // half_dt = dt/2 (0: no velocity update); ctl->chain: + next drift
 int launch_kick_drift(md_system *s, double dt, const StepCtl &ctl);

@@ -229,75 +229,94 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     m_out -= (put && !in) ? 1 : 0;
     n_lost += (acc && !put) ? 1 : 0;
   };
-  for (int ox = -1; ox <= 1; ++ox) {
-    int jx = cx + ox;
-    double sx = 0.0; unsigned kx = 0;
-    if (jx < 0) { jx += ncx; sx = -L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = L[0]; kx = 1; }
-    for (int oy = -1; oy <= 1; ++oy) {
-      int jy = cy + oy;
-      double sy = 0.0; unsigned ky = 0;
-      if (jy < 0) { jy += ncy; sy = -L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = L[1]; ky = 1; }
-      const int col = box * s.tnc + (jx * ncy + jy) * ncz;
-      // up to three runs: the in-range z cells, plus the wrapped cell on either side
-      for (int run = 0; run < 3; ++run) {
-        int c0, c1;
-        double sz = 0.0; unsigned kz = 0;
-        if (run == 0) { c0 = col + zlo; c1 = col + zhi; }
-        else if (run == 1) { if (cz - 1 >= 0) continue; c0 = c1 = col + ncz - 1; sz = -L[2]; kz = 2; }
-        else { if (cz + 1 <= ncz - 1) continue; c0 = c1 = col; sz = L[2]; kz = 1; }
-        const int jbeg = s.cell_start[c0], jend = s.cell_start[c1 + 1];
-        if (PERCELL) {
-          // four candidates per trip: the four loads are issued together (read-only path, so the list stores
-          // in between cannot hold them back), then the four tests
-          const unsigned code = kx | (ky << 2) | (kz << 4);
-          // runs across the box boundary add the shift (d + (-L) == d - L bit for bit); the others (95 % in a large box) do not
-          auto scan = [&](auto shifted) {
-            auto dist2 = [&](const double4 &pj, double &r2) {
-              double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
-              if (decltype(shifted)::value) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
-              r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            };
-            int j = jbeg;
-            for (; j + 4 <= jend; j += 4) {
-              const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
-              double r0, r1, r2, r3;
-              dist2(p0, r0); dist2(p1, r1); dist2(p2, r2); dist2(p3, r3);
-              test_keep(j, r0, code); test_keep(j + 1, r1, code); test_keep(j + 2, r2, code); test_keep(j + 3, r3, code);
-            }
-            for (; j < jend; ++j) {
-              double r2;
-              dist2(ld_pos(s.pos + j), r2);
-              test_keep(j, r2, code);
-            }
-          };
-          if (code) scan(std::true_type{}); else scan(std::false_type{});
-        } else {
-          // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
-          auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
-            unsigned ax, ay, az;
-            const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
-            const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
-            const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
-            r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            code = ax | (ay << 2) | (az << 4);
-          };
-          int j = jbeg;
-          for (; j + 4 <= jend; j += 4) {
-            const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
-            double r0, r1, r2, r3;
-            unsigned c0, c1, c2, c3;
-            dist2m(p0, r0, c0); dist2m(p1, r1, c1); dist2m(p2, r2, c2); dist2m(p3, r3, c3);
-            test_keep(j, r0, c0); test_keep(j + 1, r1, c1); test_keep(j + 2, r2, c2); test_keep(j + 3, r3, c3);
-          }
-          for (; j < jend; ++j) {
-            double r2;
-            unsigned c;
-            dist2m(ld_pos(s.pos + j), r2, c);
-            test_keep(j, r2, c);
-          }
+  // candidates of the slot range [jbeg, jend), all with the same periodic shift (sx, sy, sz) / image code
+  auto scan_range = [&](int jbeg, int jend, double sx, double sy, double sz, unsigned code) {
+    if (PERCELL) {
+      // four candidates per trip: the four loads are issued together (read-only path, so the list stores
+      // in between cannot hold them back), then the four tests
+      // runs across the box boundary add the shift (d + (-L) == d - L bit for bit); the others (95 % in a large box) do not
+      auto scan = [&](auto shifted) {
+        auto dist2 = [&](const double4 &pj, double &r2) {
+          double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
+          if (decltype(shifted)::value) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
+          r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        };
+        int j = jbeg;
+        for (; j + 4 <= jend; j += 4) {
+          const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
+          double r0, r1, r2, r3;
+          dist2(p0, r0); dist2(p1, r1); dist2(p2, r2); dist2(p3, r3);
+          test_keep(j, r0, code); test_keep(j + 1, r1, code); test_keep(j + 2, r2, code); test_keep(j + 3, r3, code);
         }
+        for (; j < jend; ++j) {
+          double r2;
+          dist2(ld_pos(s.pos + j), r2);
+          test_keep(j, r2, code);
+        }
+      };
+      if (code) scan(std::true_type{}); else scan(std::false_type{});
+    } else {
+      // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
+      auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
+        unsigned ax, ay, az;
+        const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
+        const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
+        const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
+        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        code = ax | (ay << 2) | (az << 4);
+      };
+      int j = jbeg;
+      for (; j + 4 <= jend; j += 4) {
+        const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
+        double r0, r1, r2, r3;
+        unsigned c0, c1, c2, c3;
+        dist2m(p0, r0, c0); dist2m(p1, r1, c1); dist2m(p2, r2, c2); dist2m(p3, r3, c3);
+        test_keep(j, r0, c0); test_keep(j + 1, r1, c1); test_keep(j + 2, r2, c2); test_keep(j + 3, r3, c3);
+      }
+      for (; j < jend; ++j) {
+        double r2;
+        unsigned c;
+        dist2m(ld_pos(s.pos + j), r2, c);
+        test_keep(j, r2, c);
       }
     }
+  };
+  // One (x, y) column of the stencil: up to three runs of slots: the in-range z cells (contiguous), plus the wrapped cell
+  // on either side.  part 0: all of it; part 1 / 2 (the atom's own column): the slots ABOVE / BELOW the atom's own.
+  auto column = [&](int ox, int oy, int part) {
+    int jx = cx + ox, jy = cy + oy;
+    double sx = 0.0, sy = 0.0; unsigned kx = 0, ky = 0;
+    if (jx < 0) { jx += ncx; sx = -L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = L[0]; kx = 1; }
+    if (jy < 0) { jy += ncy; sy = -L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = L[1]; ky = 1; }
+    const int col = box * s.tnc + (jx * ncy + jy) * ncz;
+    const unsigned kxy = kx | (ky << 2);
+    for (int run = 0; run < 3; ++run) {                                       // one copy of the candidate loop
+      int jbeg, jend;
+      double sz = 0.0; unsigned kz = 0;
+      if (run == 0) {                                                         // wrapped cell above
+        if (part == 2 || cz + 1 <= ncz - 1) continue;
+        jbeg = s.cell_start[col]; jend = s.cell_start[col + 1]; sz = L[2]; kz = 1;
+      } else if (run == 1) {                                                  // the in-range z cells
+        jbeg = s.cell_start[col + zlo]; jend = s.cell_start[col + zhi + 1];
+        if (part == 1) jbeg = max(jbeg, i + 1);
+        if (part == 2) jend = min(jend, i);
+      } else {                                                                // wrapped cell below
+        if (part == 1 || cz - 1 >= 0) continue;
+        jbeg = s.cell_start[col + ncz - 1]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
+      }
+      scan_range(jbeg, jend, sx, sy, sz, kxy | (kz << 4));
+    }
+  };
+  // Scan order = ownership order (row f2, Newton's third law): first the half of the stencil whose pairs THIS atom owns
+  // (columns (+1, *), (0, +1), and the slots above its own in its own column), then the other half.  Seen from the
+  // partner the offsets are negated, so exactly one atom of every pair owns it, and a row holds its owned pairs first
+  // in both of its parts without any sorting: n_own_in / n_own_out are the fill levels at the switch.
+  int n_own_in = 0, n_own_out = 0;
+  for (int c = 0; c < 10; ++c) {
+    const int ox = c < 3 ? 1 : (c < 7 ? 0 : -1);
+    const int oy = c < 3 ? 1 - c : (c == 3 ? 1 : (c == 6 ? -1 : (c < 7 ? 0 : 8 - c)));
+    if (c == 5) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
+    column(ox, oy, c == 4 ? 1 : (c == 5 ? 2 : 0));
   }
   n_out = s.cap - 1 - m_out;
   n_all += n_in + n_out + n_lost;
@@ -307,6 +326,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   for (int k = n_in; k < min((n_in + 3) & ~3, first_out); ++k) row[nbr_entry(k)] = 0u;
   for (int k = max(first_out & ~3, n_in); k < first_out; ++k) row[nbr_entry(k)] = 0u;
   s.ncount[i] = n_in | (n_out << 16);
+  s.nown[i] = n_own_in | (n_own_out << 16);
   // statistics: one atomic per warp
   const unsigned act = __activemask();
   const int wsum = __reduce_add_sync(act, n_in + n_out), wmax = __reduce_max_sync(act, n_all);

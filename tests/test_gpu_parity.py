@@ -210,6 +210,51 @@ def test_graph_step_equals_plain_launches(md, case):
     assert np.array_equal(a.positions(), b.positions())
 
 
+@pytest.mark.parametrize("half", [1, 2, 3])
+@pytest.mark.parametrize("case", ["cfg0_perm", "cfg1_small", "cfg2_small", "cfg3a_small", "cfg3b_small", "cfg4_small", "noncubic",
+                                  "alloy_tbsma_boxes", "alloy_tables_rcut", "alloy4_tbsma_boxes_rcut", "alloy3_tables", "born_mayer",
+                                  "tbsma_xi0_cross", "cfg1_rhomax_mid"])
+def test_half_list_passes(md, case, half):
+    """Row f2, Newton's third law: every undirected pair evaluated once, by the atom that owns it; the
+    partner's share arrives by 64-bit integer reductions.  Density pass (1), force pass (2) or both (3) against the
+    full-list oracle, same tolerances; bit-identical from run to run; the list itself is unchanged as a set."""
+    w = CASES[case]()
+    o = oracle_of(w)
+    of, oe, ow = o.compute_forces()
+    orho, ofp = o.densities()
+
+    def run():
+        g = md.MDSystem(w)
+        g.set_option(md.MD_OPT_FORCE_VARIANT, 1)            # half passes need one thread per atom
+        g.set_option(md.MD_OPT_HALF_LIST, half)
+        gf, ge, gw = g.compute_forces()
+        grho, gfp = g.densities()
+        g.step(30, w.dt)
+        return g, gf, ge, gw, grho, gfp, g.positions(), g.velocities()
+
+    g, gf, ge, gw, grho, gfp, gx, gv = run()
+    assert np.abs(grho - orho).max() <= 1e-12 * np.abs(orho).max()
+    assert np.abs(gfp - ofp).max() <= 1e-12 * np.abs(ofp).max()
+    assert np.abs(gf - of).max() <= F_TOL
+    assert np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    assert np.abs(gw - ow).max() <= 1e-11 * np.abs(ow).max()
+    o.step(30, w.dt)
+    d = gx - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+    g.build_neighbors()
+    o2 = oracle_of(w, positions=g.positions())
+    o2.build_neighbors()
+    assert np.array_equal(g.neighbors(192)[1], o2.neighbors(192)[1])
+    _, gf2, ge2, gw2, _, _, gx2, gv2 = run()
+    assert np.array_equal(gf, gf2) and np.array_equal(ge, ge2) and np.array_equal(gw, gw2)
+    assert np.array_equal(gx, gx2) and np.array_equal(gv, gv2)
+    # switching the option off again gives back the full-list passes
+    g.set_option(md.MD_OPT_HALF_LIST, 0)
+    gf3 = g.compute_forces()[0]
+    assert np.abs(gf3 - oracle_of(w, positions=g.positions()).compute_forces()[0]).max() <= F_TOL
+
+
 @pytest.mark.parametrize("case", ["cfg0", "cfg2_small", "cfg4_small", "alloy_tables_rcut"])
 @pytest.mark.parametrize("graph", [1, 0])
 def test_chained_steps_equal_single_steps(md, case, graph):
