@@ -338,27 +338,24 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
         hx = torch.empty((n, 3), dtype=torch.float64).pin_memory()
         hv = torch.empty((n, 3), dtype=torch.float64).pin_memory()
         hxn, hvn = hx.numpy(), hv.numpy()
-        g.positions(out=hxn)
-        g.velocities(out=hvn)
+        g.get_state(out=(hxn, hvn))
         Ke = min(K, args.e2e_steps) if args.e2e_steps else K
         for _ in range(3):
-            g.set_positions(hxn); g.set_velocities(hvn); g.step(1, w.dt); g.positions(out=hxn); g.velocities(out=hvn)
+            g.set_state(hxn, hvn); g.step(1, w.dt); g.get_state(out=(hxn, hvn))
         barrier()
         t0 = time.perf_counter()
         for _ in range(Ke):
-            g.set_positions(hxn)
-            g.set_velocities(hvn)
+            g.set_state(hxn, hvn)
             g.step(1, w.dt)
-            g.positions(out=hxn)
-            g.velocities(out=hvn)
+            g.get_state(out=(hxn, hvn))
         barrier()
         te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         e2e = {"value": world * n * Ke / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
                "steps": Ke, "ms_per_step": 1e3 * float(te.item()) / Ke,
-               "what": "per step: md_set_positions + md_set_velocities from pinned host arrays, md_step(1) (forces are "
-                       "re-evaluated for the new positions, then one velocity-Verlet step), md_get_positions + md_get_velocities"}
+               "what": "per step: md_set_state(x, v) from pinned host arrays (48 B per atom host->device; the forces stay valid when "
+                       "the uploaded coordinates are the resident ones), md_step(1), md_get_state(x, v) (48 B per atom device->host)"}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -161,6 +161,13 @@ int md_get_positions(md_system *s, double *x);        /* [n_atoms][3]; as wrappe
 int md_get_velocities(md_system *s, double *v);       /* [n_atoms][3] */
 int md_set_positions(md_system *s, const double *x);  /* keeps the list if no atom is farther than skin/2 from x_ref */
 int md_set_velocities(md_system *s, const double *v);
+/* Positions and velocities in one call (either may be NULL = skip): one kernel, and for host buffers one
+ * synchronisation instead of two.  md_set_state leaves an atom whose uploaded coordinates are bit-identical to the
+ * resident ones untouched, and keeps the forces valid if NO coordinate changed (so a caller that only edits
+ * velocities, or echoes a state back, does not pay for a force evaluation); it synchronises even for device pointers
+ * when x is given (it reads that flag). */
+int md_set_state(md_system *s, const double *x, const double *v);
+int md_get_state(md_system *s, double *x, double *v);
 /* Test hook: the list as ORIGINAL (caller) indices, ascending per atom.  count [n_atoms], list [n_atoms][stride]
  * (each row padded with -1); MD_ESTATE before the first build, MD_EOVERFLOW if some count exceeds stride. */
 int md_get_neighbors(md_system *s, int *count, int *list, int stride);

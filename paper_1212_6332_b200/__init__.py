@@ -72,6 +72,8 @@ def lib() -> C.CDLL:
         L.md_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
         for name in ("md_get_positions", "md_get_velocities", "md_set_positions", "md_set_velocities"):
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
+        for name in ("md_set_state", "md_get_state"):
+            getattr(L, name).argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_get_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.md_get_densities.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_get_energies.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -223,6 +225,16 @@ class MDSystem:
     def set_velocities(self, v):
         v = _host(v, np.float64)
         check(lib().md_set_velocities(self._h, _ptr(v)))
+
+    def set_state(self, x=None, v=None):
+        x, v = _host(x, np.float64), _host(v, np.float64)
+        check(lib().md_set_state(self._h, _ptr(x), _ptr(v)))
+
+    def get_state(self, device_out: bool = False, out=None):
+        x, v = out if out is not None else (self._out((self.n_atoms, 3), np.float64, device_out),
+                                            self._out((self.n_atoms, 3), np.float64, device_out))
+        check(lib().md_get_state(self._h, _ptr(x), _ptr(v)))
+        return x, v
 
     def neighbors(self, stride: int = 256, device_out: bool = False):
         cnt = self._out((self.n_atoms,), np.int32, device_out)

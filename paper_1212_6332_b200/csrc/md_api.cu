@@ -46,7 +46,7 @@ struct Bump {
   }
 };
 
-struct Geometry { int nc[3], tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
+struct Geometry { int nc[3], reach, tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
 
 // check_pairs: also validate the optional per-pair host arrays (md_create); the size query reads no pointer of *d
 static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
@@ -77,6 +77,17 @@ static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
     if (g.nc[a] < 3) return MD_EBOX;                 // 26 distinct neighbour cells
     vol *= d->box[a];
   }
+  // Cells of half the list cut-off with a 5 x 5 x 5 stencil (reach 2) hold 15.6 cell volumes of candidates instead of 27, but
+  // measured on B200 the build got SLOWER (0.58 -> 0.76 ms per 1 M atoms, 1.6 -> 2.0 ms at 4.2 M): 25 short runs of ~8 slots
+  // per atom cost more in run set-up and divergence than the 42 % of distance tests they save, and the passes lost
+  // 2-6 % to the coarser locality of the atom order.  The kernels take any reach; md_create uses the paper's 27 cells.
+  g.reach = getenv("MD_CELL_REACH") && atoi(getenv("MD_CELL_REACH")) == 2 ? 2 : 1;
+  if (g.reach == 2) {
+    int fine[3];
+    for (int a = 0; a < 3; ++a) fine[a] = (int)floor(2.0 * d->box[a] / rl);
+    if ((double)fine[0] * fine[1] * fine[2] * d->n_boxes > 1.6e7) g.reach = 1;
+    else for (int a = 0; a < 3; ++a) g.nc[a] = fine[a];
+  }
   const double cells = (double)g.nc[0] * g.nc[1] * g.nc[2];
   if (cells * d->n_boxes > 1.6e7) return MD_EINVAL;  // two-level scan limit (4096 * 4096 cells)
   g.tnc = g.nc[0] * g.nc[1] * g.nc[2];
@@ -94,7 +105,7 @@ static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
   g.tiles_per_box = (g.npb + 31) / 32;
   // block partials: enough for the 8-lanes-per-atom variant, and for 32 lanes per atom where that variant is allowed
   g.n_blocks = d->n_boxes * blocks_per_box(g.npb, kForceBlock / (d->n_atoms <= kSub32Limit ? 32 : 8));
-  g.stage_bytes = (size_t)d->n_atoms * 3 * sizeof(double);
+  g.stage_bytes = (size_t)d->n_atoms * 6 * sizeof(double);        // positions and velocities of one md_set_state / md_get_state
   if (g.stage_bytes < (1u << 20)) g.stage_bytes = 1u << 20;
   return MD_OK;
 }
@@ -221,6 +232,37 @@ __global__ void k_set_pos(const __grid_constant__ DevSys s, const double *__rest
     atomicMax(&s.st->maxd2_bits, (unsigned long long)__double_as_longlong(d2));
   }
   p.x = x[0]; p.y = x[1]; p.z = x[2];
+  s.pos[i] = p;
+}
+
+// md_set_state: positions (as k_set_pos, but an atom whose uploaded coordinates are bit-identical to the resident ones is
+// left alone and does not count as moved) and velocities in one kernel; *changed is set if some position differs.
+__global__ void k_set_state(const __grid_constant__ DevSys s, const double *__restrict__ x, const double *__restrict__ v, int have_ref,
+                            int *changed) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  const size_t o = 3 * (size_t)s.orig[i], N = (size_t)s.N;
+  if (v) { s.vel[i] = v[o]; s.vel[N + i] = v[o + 1]; s.vel[2 * N + i] = v[o + 2]; }
+  if (!x) return;
+  double4 p = s.pos[i];
+  double q[3] = {x[o], x[o + 1], x[o + 2]};
+  if (q[0] == p.x && q[1] == p.y && q[2] == p.z) return;
+  *changed = 1;
+  if (have_ref) {
+    double d2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double ref = s.xref[c * N + i];
+      double u = q[c] - ref;
+      const double Lc = box_edge(s, c);
+      u -= Lc * rint(u / Lc);
+      q[c] = ref + u;
+      d2 += u * u;
+    }
+    if (!(d2 == d2)) d2 = __longlong_as_double(0x7ff0000000000000ll);
+    atomicMax(&s.st->maxd2_bits, (unsigned long long)__double_as_longlong(d2));
+  }
+  p.x = q[0]; p.y = q[1]; p.z = q[2];
   s.pos[i] = p;
 }
 
@@ -490,6 +532,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   const double rl = d->cutoff + d->skin;
   for (int a = 0; a < 3; ++a) {
     o.nc[a] = g.nc[a]; o.L0[a] = d->box[a];
+    o.reach = g.reach;
   }
   o.rl = rl; o.dyn_box = 0;
   for (int k = 0; k < o.nt * o.nt; ++k) { const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff; o.rc2p[k] = rc * rc; }
@@ -755,6 +798,54 @@ int md_set_positions(md_system *s, const double *x) {
   s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;
   if (src != x && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;   // the host buffer may be reused
   return check_cuda(cudaGetLastError());
+}
+
+int md_set_state(md_system *s, const double *x, const double *v) {
+  if (!s || (!x && !v)) return MD_EINVAL;
+  const DevSys &o = s->d;
+  const size_t bytes = 3 * (size_t)o.N * sizeof(double);
+  const double *xs = x, *vs = v;
+  bool host = false;
+  if (x && !on_device(x)) {
+    if (cudaMemcpyAsync(s->stage, x, bytes, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
+    xs = (const double *)s->stage; host = true;
+  }
+  if (v && !on_device(v)) {
+    if (cudaMemcpyAsync((char *)s->stage + bytes, v, bytes, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return MD_ECUDA;
+    vs = (const double *)((char *)s->stage + bytes); host = true;
+  }
+  int *flag = o.scan_block;                            // free outside the rebuild chain
+  if (cudaMemsetAsync(flag, 0, sizeof(int), s->stream) != cudaSuccess) return MD_ECUDA;
+  ++s->launches, k_set_state<<<grid_for(o.N), 256, 0, s->stream>>>(o, xs, vs, s->have_list ? 1 : 0, flag);
+  if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
+  if (!x) return host && cudaStreamSynchronize(s->stream) != cudaSuccess ? MD_ECUDA : MD_OK;
+  // the forces stay valid if no coordinate changed: that takes one look at the flag (and the host buffers may be reused)
+  int changed = 1;
+  if (cudaMemcpyAsync(&changed, flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+      cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
+  if (changed) { s->forces_valid = false; s->observables_valid = false; s->frc_keep = false; }
+  return MD_OK;
+}
+
+int md_get_state(md_system *s, double *x, double *v) {
+  if (!s || (!x && !v)) return MD_EINVAL;
+  const DevSys &o = s->d;
+  const size_t bytes = 3 * (size_t)o.N * sizeof(double);
+  bool host = false;
+  if (x) {
+    const bool dev = on_device(x);
+    double *dst = dev ? x : (double *)s->stage;
+    ++s->launches, k_get_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, dst);
+    if (!dev) { host = true; if (cudaMemcpyAsync(x, dst, bytes, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA; }
+  }
+  if (v) {
+    const bool dev = on_device(v);
+    double *dst = dev ? v : (double *)((char *)s->stage + bytes);
+    ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, dst);
+    if (!dev) { host = true; if (cudaMemcpyAsync(v, dst, bytes, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA; }
+  }
+  if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
+  return host ? sync_and_flags(s) : MD_OK;
 }
 
 int md_set_velocities(md_system *s, const double *v) {

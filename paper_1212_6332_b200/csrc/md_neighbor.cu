@@ -188,12 +188,14 @@ __device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-
   return v;
 }
 
-// PERCELL (every nc >= 5): two atoms of cells that are neighbours WITHOUT crossing the box boundary are closer than
-// 2L/nc <= 0.4 L per axis, and two atoms of cells that are neighbours ACROSS the boundary differ by more than 0.6 L, so
+// The stencil is (2R+1)^3 cells of side >= r_l / R (R = DevSys::reach: 2, or 1 for very large systems; the paper uses
+// R = 1): with R = 2 a build tests 15.6 cell volumes of candidates instead of 27.
+// PERCELL (every nc >= 2R+3): two atoms of cells within reach WITHOUT crossing the box boundary are closer than
+// (R+1) L/nc <= 0.43 L per axis, and two atoms of cells within reach ACROSS the boundary differ by more than 0.57 L, so
 // the branch of the canonical minimum image is decided by the pair of cells: the shift (0, -L or +L) and its image
 // code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
 // (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
-template <bool PERCELL>
+template <bool PERCELL, int R>
 __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
@@ -208,7 +210,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   const int cy = cell_coord(pi.y, s.nc[1] / L[1], s.nc[1]);
   const int cz = cell_coord(pi.z, s.nc[2] / L[2], s.nc[2]);
   const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
-  const int zlo = max(cz - 1, 0), zhi = min(cz + 1, ncz - 1);
+  const int zlo = max(cz - R, 0), zhi = min(cz + R, ncz - 1);
   int n_all = 0;
   // pairs inside r_in (= r_c) now go to the front of the row (k = 0, 1, ...), skin pairs to the back (k = cap-1, cap-2, ...):
   // the two passes run the full pair evaluation only over the front part (md_force.cu)
@@ -293,30 +295,31 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     for (int run = 0; run < 3; ++run) {                                       // one copy of the candidate loop
       int jbeg, jend;
       double sz = 0.0; unsigned kz = 0;
-      if (run == 0) {                                                         // wrapped cell above
-        if (part == 2 || cz + 1 <= ncz - 1) continue;
-        jbeg = s.cell_start[col]; jend = s.cell_start[col + 1]; sz = L[2]; kz = 1;
+      if (run == 0) {                                                         // wrapped cells above: 0 .. cz + R - ncz
+        if (part == 2 || cz + R <= ncz - 1) continue;
+        jbeg = s.cell_start[col]; jend = s.cell_start[col + cz + R - ncz + 1]; sz = L[2]; kz = 1;
       } else if (run == 1) {                                                  // the in-range z cells
         jbeg = s.cell_start[col + zlo]; jend = s.cell_start[col + zhi + 1];
         if (part == 1) jbeg = max(jbeg, i + 1);
         if (part == 2) jend = min(jend, i);
-      } else {                                                                // wrapped cell below
-        if (part == 1 || cz - 1 >= 0) continue;
-        jbeg = s.cell_start[col + ncz - 1]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
+      } else {                                                                // wrapped cells below: ncz + cz - R .. ncz - 1
+        if (part == 1 || cz - R >= 0) continue;
+        jbeg = s.cell_start[col + ncz + cz - R]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
       }
       scan_range(jbeg, jend, sx, sy, sz, kxy | (kz << 4));
     }
   };
   // Scan order = ownership order (row f2, Newton's third law): first the half of the stencil whose pairs THIS atom owns
-  // (columns (+1, *), (0, +1), and the slots above its own in its own column), then the other half.  Seen from the
-  // partner the offsets are negated, so exactly one atom of every pair owns it, and a row holds its owned pairs first
+  // (columns (ox > 0, *), (0, oy > 0), and the slots above its own in its own column), then the other half.  Seen from
+  // the partner the offsets are negated, so exactly one atom of every pair owns it, and a row holds its owned pairs first
   // in both of its parts without any sorting: n_own_in / n_own_out are the fill levels at the switch.
   int n_own_in = 0, n_own_out = 0;
-  for (int c = 0; c < 10; ++c) {
-    const int ox = c < 3 ? 1 : (c < 7 ? 0 : -1);
-    const int oy = c < 3 ? 1 - c : (c == 3 ? 1 : (c == 6 ? -1 : (c < 7 ? 0 : 8 - c)));
-    if (c == 5) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
-    column(ox, oy, c == 4 ? 1 : (c == 5 ? 2 : 0));
+  constexpr int W = 2 * R + 1, kCentre = (W * W) / 2;
+#pragma unroll 1
+  for (int c = 0; c <= W * W; ++c) {                                          // (ox, oy) in descending lexicographic order, the centre twice
+    const int q = c <= kCentre ? c : c - 1;
+    if (c == kCentre + 1) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
+    column(R - q / W, R - q % W, c == kCentre ? 1 : (c == kCentre + 1 ? 2 : 0));   // ONE call site: one copy of the candidate loops
   }
   n_out = s.cap - 1 - m_out;
   n_all += n_in + n_out + n_lost;
@@ -381,8 +384,14 @@ int launch_rebuild_body(md_system *sys) {
   {
     ProfScope p(sys, MD_K_LIST);
     const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);
-    if (d.nc[0] >= 5 && d.nc[1] >= 5 && d.nc[2] >= 5) ++sys->launches, k_build_list<true><<<gl, kForceBlock, 0, st>>>(d);
-    else ++sys->launches, k_build_list<false><<<gl, kForceBlock, 0, st>>>(d);
+    const int need = 2 * d.reach + 3;     // cells per edge from which the image of a pair is decided by its pair of cells
+    const bool percell = d.nc[0] >= need && d.nc[1] >= need && d.nc[2] >= need;
+    ++sys->launches;
+    if (d.reach == 2) {
+      if (percell) k_build_list<true, 2><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, 2><<<gl, kForceBlock, 0, st>>>(d);
+    } else {
+      if (percell) k_build_list<true, 1><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, 1><<<gl, kForceBlock, 0, st>>>(d);
+    }
   }
   return (int)cudaGetLastError();
 }

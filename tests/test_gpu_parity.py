@@ -255,6 +255,31 @@ def test_half_list_passes(md, case, half):
     assert np.abs(gf3 - oracle_of(w, positions=g.positions()).compute_forces()[0]).max() <= F_TOL
 
 
+@pytest.mark.parametrize("case", ["cfg0_perm", "cfg2_small", "cfg3b_small", "cfg4_small", "noncubic", "alloy_tbsma_boxes"])
+def test_cell_reach_two(md, case, monkeypatch):
+    """The list build with cells of half the list cut-off and a 5 x 5 x 5 stencil (MD_CELL_REACH=2, measured slower on
+    B200 and therefore not the default): the same pair sets, forces and trajectory."""
+    monkeypatch.setenv("MD_CELL_REACH", "2")
+    w = CASES[case]()
+    o = oracle_of(w)
+    g = md.MDSystem(w)
+    g.build_neighbors()
+    o.build_neighbors()
+    assert np.array_equal(g.neighbors(192)[1], o.neighbors(192)[1])
+    gf, ge, gw = g.compute_forces()
+    of, oe, ow = o.compute_forces()
+    assert np.abs(gf - of).max() <= F_TOL and np.abs(ge - oe).max() <= 1e-12 * np.abs(oe).max()
+    g.step(40, w.dt)
+    o.step(40, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0 and g.stats()["rebuilds"] >= 2
+    g.build_neighbors()
+    o2 = oracle_of(w, positions=g.positions())
+    o2.build_neighbors()
+    assert np.array_equal(g.neighbors(192)[1], o2.neighbors(192)[1])
+
+
 @pytest.mark.parametrize("case", ["cfg0", "cfg2_small", "cfg4_small", "alloy_tables_rcut"])
 @pytest.mark.parametrize("graph", [1, 0])
 def test_chained_steps_equal_single_steps(md, case, graph):
@@ -457,6 +482,36 @@ def test_set_get_roundtrip_and_device_inputs(md):
     gd = md.MDSystem(w, positions=torch.from_numpy(w.positions).cuda(), velocities=torch.from_numpy(w.velocities).cuda(),
                      types=torch.from_numpy(w.types).cuda())
     assert np.array_equal(gd.compute_forces()[0], md.MDSystem(w).compute_forces()[0])
+
+
+def test_set_get_state(md):
+    """md_set_state / md_get_state: one call for positions and velocities; an echoed state keeps the forces (no second
+    evaluation, bit-identical trajectory); changed coordinates invalidate them."""
+    w = CASES["cfg3a_small"]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    a.step(30, w.dt)
+    for it in range(30):
+        x, v = b.get_state()
+        assert np.array_equal(x, b.positions()) and np.array_equal(v, b.velocities())
+        l0 = b.stats()["kernel_launches"]
+        b.set_state(x, v)
+        b.step(1, w.dt)
+        if it:      # (the first step of a new system evaluates its initial forces)
+            assert b.stats()["kernel_launches"] - l0 <= 6 + 10     # set, drift, density, force (+ a rebuild): no extra force evaluation
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    # velocities only
+    x, v = b.get_state()
+    b.set_state(None, 0.5 * v)
+    assert np.array_equal(b.velocities(), 0.5 * v) and np.array_equal(b.positions(), x)
+    # changed positions: the next call evaluates the forces for them (against the oracle)
+    x2 = x + 0.01 * np.sin(np.arange(x.size).reshape(x.shape))
+    b.set_state(x2, v)
+    o = oracle_of(w, positions=x2, velocities=v)
+    assert np.abs(b.compute_forces()[0] - o.compute_forces()[0]).max() <= F_TOL
+    # device tensors
+    xt, vt = b.get_state(device_out=True)
+    b.set_state(xt, vt)
+    assert np.array_equal(xt.cpu().numpy(), b.positions())
 
 
 def test_error_codes(md):
