@@ -219,6 +219,13 @@ const char *md_kernel_name(int kernel_class);
  * the call) and synchronises the device. */
 int md_fp64_dfma_rate(void *stream, double *dfma_per_s, double *sm_clock_mhz);
 
+/* Diagnostic: time per warp-wide gather of 32-byte table records (ns, one SM serving 32 resident warps), the access that
+ * binds the table passes, in four forms: [0] table in global memory through L1, indices distributed as the passes see
+ * them (what the passes do); [1] the reachable window of the table staged in shared memory, same indices; [2], [3] the
+ * same two with interval-sorted indices (32 adjacent records per warp).  Not part of the MD path; allocates 160 KB
+ * (cudaMalloc / cudaFree inside the call) and synchronises the stream. */
+int md_probe_table_gather(void *stream, double ns_per_warp_gather[4]);
+
 const char *md_strerror(int status);
 const char *md_version(void);
 

@@ -122,6 +122,14 @@ def fp64_dfma_rate():
     return rate.value, mhz.value
 
 
+def probe_table_gather():
+    """ns per warp-wide gather of 32-byte table records: (global random, shared random, global sorted, shared sorted)."""
+    import torch
+    out = (C.c_double * 4)()
+    check(lib().md_probe_table_gather(C.c_void_p(torch.cuda.current_stream().cuda_stream), out))
+    return tuple(out)
+
+
 class MDSystem:
     """One system on the current CUDA device.  `w` is a workloads.Workload (or pass the same fields by keyword).
     Array arguments may be numpy arrays (host) or torch CUDA tensors (device)."""

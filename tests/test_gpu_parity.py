@@ -514,6 +514,13 @@ def test_set_get_state(md):
     assert np.array_equal(xt.cpu().numpy(), b.positions())
 
 
+def test_diagnostics_run(md):
+    rate, mhz = md.fp64_dfma_rate()
+    assert rate > 1e12 and mhz > 500
+    g = md.probe_table_gather()
+    assert len(g) == 4 and all(0.5 < v < 1e4 for v in g)
+
+
 def test_error_codes(md):
     w = workloads.config(0, scale=4)             # L = 14.46 < 3 * 5.2
     with pytest.raises(md.MDError) as ei:
