@@ -115,7 +115,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   DevSys t;  // filled only when sys != nullptr
   const size_t N = (size_t)d->n_atoms, nt2 = (size_t)d->n_types * d->n_types;
   t.st = b.take<DevState>(1);
-  t.pos = b.take<double4>(N); t.posf = b.take<double4>(N); t.pos_tmp = b.take<double4>(N);
+  t.pos = b.take<double4>(N); t.posf = b.take<double4>(N); t.pos_tmp = b.take<double4>(N); t.pos32 = b.take<float4>(N);
   t.vel = b.take<double>(3 * N); t.vel_tmp = b.take<double>(3 * N);
   t.frc = b.take<double>(3 * N); t.xref = b.take<double>(3 * N);
   t.type = b.take<int>(N); t.type_tmp = b.take<int>(N); t.orig = b.take<int>(N); t.orig_tmp = b.take<int>(N);
@@ -142,7 +142,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   void *stage = b.take<char>(g.stage_bytes);
   if (sys) {
     DevSys &o = sys->d;
-    o.st = t.st; o.pos = t.pos; o.posf = t.posf; o.pos_tmp = t.pos_tmp; o.vel = t.vel; o.vel_tmp = t.vel_tmp;
+    o.st = t.st; o.pos = t.pos; o.posf = t.posf; o.pos_tmp = t.pos_tmp; o.pos32 = t.pos32; o.vel = t.vel; o.vel_tmp = t.vel_tmp;
     o.frc = t.frc; o.xref = t.xref; o.type = t.type; o.type_tmp = t.type_tmp; o.orig = t.orig; o.orig_tmp = t.orig_tmp;
     o.cell_id = t.cell_id; o.perm = t.perm; o.cell_count = t.cell_count; o.cell_start = t.cell_start;
     o.cell_fill = t.cell_fill; o.scan_block = t.scan_block; o.nbr = t.nbr; o.ncount = t.ncount; o.rho = t.rho;

@@ -162,6 +162,7 @@ __global__ void k_copyback(const __grid_constant__ DevSys s) {
   if (i >= s.N) return;
   const double4 p = s.pos_tmp[i];
   s.pos[i] = p;
+  s.pos32[i] = make_float4((float)p.x, (float)p.y, (float)p.z, 0.f);                     // the list build's first look at a candidate
   s.xref[i] = p.x; s.xref[(size_t)s.N + i] = p.y; s.xref[2 * (size_t)s.N + i] = p.z;   // x_ref <- x
 #pragma unroll
   for (int c = 0; c < 3; ++c) s.vel[(size_t)c * s.N + i] = s.vel_tmp[(size_t)c * s.N + i];
@@ -285,7 +286,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   };
   // One (x, y) column of the stencil: up to three runs of slots: the in-range z cells (contiguous), plus the wrapped cell
   // on either side.  part 0: all of it; part 1 / 2 (the atom's own column): the slots ABOVE / BELOW the atom's own.
-  auto column = [&](int ox, int oy, int part) {
+  auto column = [&](int ox, int oy, int part, auto &&range) {
     int jx = cx + ox, jy = cy + oy;
     double sx = 0.0, sy = 0.0; unsigned kx = 0, ky = 0;
     if (jx < 0) { jx += ncx; sx = -L[0]; kx = 2; } else if (jx >= ncx) { jx -= ncx; sx = L[0]; kx = 1; }
@@ -306,20 +307,108 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
         if (part == 1 || cz - R >= 0) continue;
         jbeg = s.cell_start[col + ncz + cz - R]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
       }
-      scan_range(jbeg, jend, sx, sy, sz, kxy | (kz << 4));
+      range(jbeg, jend, sx, sy, sz, kxy | (kz << 4));
     }
   };
   // Scan order = ownership order (row f2, Newton's third law): first the half of the stencil whose pairs THIS atom owns
   // (columns (ox > 0, *), (0, oy > 0), and the slots above its own in its own column), then the other half.  Seen from
   // the partner the offsets are negated, so exactly one atom of every pair owns it, and a row holds its owned pairs first
-  // in both of its parts without any sorting: n_own_in / n_own_out are the fill levels at the switch.
-  int n_own_in = 0, n_own_out = 0;
-  constexpr int W = 2 * R + 1, kCentre = (W * W) / 2;
+  // in both of its parts without any sorting: at_switch() notes the fill levels between the two halves.
+  auto stencil = [&](auto &&range, auto &&at_switch) {
+    constexpr int W = 2 * R + 1, kCentre = (W * W) / 2;
 #pragma unroll 1
-  for (int c = 0; c <= W * W; ++c) {                                          // (ox, oy) in descending lexicographic order, the centre twice
-    const int q = c <= kCentre ? c : c - 1;
-    if (c == kCentre + 1) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
-    column(R - q / W, R - q % W, c == kCentre ? 1 : (c == kCentre + 1 ? 2 : 0));   // ONE call site: one copy of the candidate loops
+    for (int c = 0; c <= W * W; ++c) {                                        // (ox, oy) in descending lexicographic order, the centre twice
+      const int q = c <= kCentre ? c : c - 1;
+      if (c == kCentre + 1) at_switch();
+      column(R - q / W, R - q % W, c == kCentre ? 1 : (c == kCentre + 1 ? 2 : 0), range);   // ONE call site: one copy of the candidate loop
+    }
+  };
+  int n_own_in = 0, n_own_out = 0;
+
+  // ---- Phase 1: single-precision filter.  9 of 10 candidates of the 27 cells are beyond r_l; they are rejected on float
+  // copies of the coordinates (pos32, written with the re-order) against r_l^2 plus a margin that covers the rounding of
+  // the copies (|x| <= L: 2^-24 L per coordinate), so no pair of the list can be missed.  The survivors (the list plus
+  // about one candidate in 10^4) are parked in the row itself, in scan order.
+  const float4 q32 = s.pos32[i];
+  const float Lf[3] = {(float)L[0], (float)L[1], (float)L[2]}, iLf[3] = {1.f / Lf[0], 1.f / Lf[1], 1.f / Lf[2]};
+  const float rl2f = (float)s.rl2 + 4e-6f * (float)s.rl * (fmaxf(fmaxf(Lf[0], Lf[1]), Lf[2]) + (float)s.rl);
+  int ns = 0, ns_own = 0;
+  bool exact_path = false;                                        // the row cannot hold the survivors: classify during the scan instead
+  auto park = [&](int j, float r2, unsigned code) {
+    const bool hit = r2 < rl2f && j != i;
+    const bool put = hit && ns < s.cap;
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .u64 a;\n\tsetp.ne.u32 p, %3, 0;\n\tmad.wide.u32 a, %1, 4, %0;\n\t@p st.global.u32 [a], %2;\n\t}"
+                 :: "l"((unsigned long long)row), "r"(nbr_entry(ns)), "r"((unsigned)j | (code << kIdxBits)), "r"((unsigned)put) : "memory");
+    ns += put ? 1 : 0;
+    exact_path |= hit && !put;
+  };
+  auto filter_range = [&](int jbeg, int jend, double sx, double sy, double sz, unsigned code) {
+    auto ld32 = [&](int j) {
+      float4 v;
+      asm("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(s.pos32 + j));
+      return v;
+    };
+    const float fx = (float)sx, fy = (float)sy, fz = (float)sz;
+    auto dist2f = [&](const float4 &a) {
+      float dx = a.x - q32.x, dy = a.y - q32.y, dz = a.z - q32.z;
+      if (PERCELL) { dx += fx; dy += fy; dz += fz; }
+      else {                                                      // nearest image: either image is beyond r_l when they tie (L >= 3 r_l)
+        dx -= Lf[0] * rintf(dx * iLf[0]); dy -= Lf[1] * rintf(dy * iLf[1]); dz -= Lf[2] * rintf(dz * iLf[2]);
+      }
+      return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    };
+    int j = jbeg;
+    for (; j + 4 <= jend; j += 4) {
+      const float4 a0 = ld32(j), a1 = ld32(j + 1), a2 = ld32(j + 2), a3 = ld32(j + 3);
+      const float r0 = dist2f(a0), r1 = dist2f(a1), r2 = dist2f(a2), r3 = dist2f(a3);
+      park(j, r0, code); park(j + 1, r1, code); park(j + 2, r2, code); park(j + 3, r3, code);
+    }
+    for (; j < jend; ++j) park(j, dist2f(ld32(j)), code);
+  };
+  // Measured on B200: a gain only where the exact test is expensive (small boxes: minimum image per pair, cfg2 list build
+  // 0.140 -> 0.094 ms per step); in large boxes (PERCELL) the scan's loads are broadcasts within a cell while the second
+  // phase gathers one position per survivor and lane, and the L1 data pipe makes the build 20 % SLOWER (0.58 -> 0.70 ms per
+  // 1 M atoms): there every candidate is classified in double precision during the scan, as in round 1.
+  if constexpr (PERCELL) exact_path = true;
+  else stencil(filter_range, [&]() { ns_own = ns; });
+
+  // ---- Phase 2: the survivors, in the same order, with the canonical double-precision test (reading A3); accepted
+  // entries go back into the row from both ends (the front never overtakes the reader)
+  if (!exact_path) {
+    for (int t = 0; t < ns; ++t) {
+      if (t == ns_own) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
+      const unsigned e = row[nbr_entry(t)];
+      const int j = (int)(e & kIdxMask);
+      const double4 pj = ld_pos(s.pos + j);
+      double r2;
+      unsigned code;
+      if (PERCELL) {
+        code = e >> kIdxBits;
+        double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
+        if (code) {                                               // the shifts of the run this candidate came from (0.0 where none)
+          dx = __dadd_rn(dx, (code & 1u) ? L[0] : ((code & 2u) ? -L[0] : 0.0));
+          dy = __dadd_rn(dy, (code & 4u) ? L[1] : ((code & 8u) ? -L[1] : 0.0));
+          dz = __dadd_rn(dz, (code & 16u) ? L[2] : ((code & 32u) ? -L[2] : 0.0));
+        }
+        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+      } else {
+        unsigned ax, ay, az;
+        const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
+        const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
+        const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
+        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        code = ax | (ay << 2) | (az << 4);
+      }
+      if (r2 < s.rl2 && !(r2 < s.rin2) && m_out > t && m_out < ns) { exact_path = true; break; }   // the back would overwrite unread survivors
+      test_keep(j, r2, code);
+    }
+    if (ns_own >= ns) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
+  }
+  // ---- Rows too full for that (a capacity close to the row length, or an overflow): every candidate classified in double
+  // precision during the scan, which also counts what does not fit
+  if (exact_path) {
+    n_in = 0; m_out = s.cap - 1; n_lost = 0;
+    stencil(scan_range, [&]() { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; });
   }
   n_out = s.cap - 1 - m_out;
   n_all += n_in + n_out + n_lost;
