@@ -46,7 +46,7 @@ struct Bump {
   }
 };
 
-struct Geometry { int nc[3], reach, tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
+struct Geometry { int nc[3], zfine, tnc, ncell, cap, tiles_per_box, n_blocks, npb; size_t stage_bytes; };
 
 // check_pairs: also validate the optional per-pair host arrays (md_create); the size query reads no pointer of *d
 static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
@@ -77,17 +77,18 @@ static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
     if (g.nc[a] < 3) return MD_EBOX;                 // 26 distinct neighbour cells
     vol *= d->box[a];
   }
-  // Cells of half the list cut-off with a 5 x 5 x 5 stencil (reach 2) hold 15.6 cell volumes of candidates instead of 27, but
-  // measured on B200 the build got SLOWER (0.58 -> 0.76 ms per 1 M atoms, 1.6 -> 2.0 ms at 4.2 M): 25 short runs of ~8 slots
-  // per atom cost more in run set-up and divergence than the 42 % of distance tests they save, and the passes lost
-  // 2-6 % to the coarser locality of the atom order.  The kernels take any reach; md_create uses the paper's 27 cells.
-  g.reach = getenv("MD_CELL_REACH") && atoi(getenv("MD_CELL_REACH")) == 2 ? 2 : 1;
-  if (g.reach == 2) {
-    int fine[3];
-    for (int a = 0; a < 3; ++a) fine[a] = (int)floor(2.0 * d->box[a] / rl);
-    if ((double)fine[0] * fine[1] * fine[2] * d->n_boxes > 1.6e7) g.reach = 1;
-    else for (int a = 0; a < 3; ++a) g.nc[a] = fine[a];
-  }
+  // Small boxes (some edge shorter than 5 r_l: the image of a pair is decided per pair, and the build filters in single
+  // precision): cells four times thinner in z (the fastest cell index: a column of cells is one contiguous run of slots).
+  // The candidates of a column are then the z window [z_i - w, z_i + w], w^2 = r_l^2 - (lateral gap to the column)^2,
+  // instead of three whole cells: cfg2 list build 0.094 -> 0.082 ms per step.  Large boxes keep cubic cells: there the
+  // lanes of a warp that share a cell scan the SAME slots (their loads are broadcasts), and per-atom windows cost more in
+  // L1 wavefronts than they save in tests (measured: 0.58 -> 0.70 ms per 1 M atoms with quarter cells, 0.61 with half).
+  // Also measured and dropped: cells of half the cut-off in all three directions with a 5 x 5 x 5 stencil (0.76 ms).
+  const bool large = g.nc[0] >= 5 && g.nc[1] >= 5 && g.nc[2] >= 5;
+  g.zfine = large ? 1 : 4;
+  if (const char *e = getenv("MD_CELL_ZFINE")) { const int v = atoi(e); if (v == 1 || v == 2 || v == 4) g.zfine = v; }   // for the measurements above
+  while (g.zfine > 1 && (double)g.nc[0] * g.nc[1] * floor(g.zfine * d->box[2] / rl) * d->n_boxes > 1.6e7) g.zfine /= 2;
+  g.nc[2] = (int)floor(g.zfine * d->box[2] / rl);
   const double cells = (double)g.nc[0] * g.nc[1] * g.nc[2];
   if (cells * d->n_boxes > 1.6e7) return MD_EINVAL;  // two-level scan limit (4096 * 4096 cells)
   g.tnc = g.nc[0] * g.nc[1] * g.nc[2];
@@ -532,7 +533,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   const double rl = d->cutoff + d->skin;
   for (int a = 0; a < 3; ++a) {
     o.nc[a] = g.nc[a]; o.L0[a] = d->box[a];
-    o.reach = g.reach;
+    o.zfine = g.zfine;
   }
   o.rl = rl; o.dyn_box = 0;
   for (int k = 0; k < o.nt * o.nt; ++k) { const double rc = d->pair_cutoff ? d->pair_cutoff[k] : d->cutoff; o.rc2p[k] = rc * rc; }

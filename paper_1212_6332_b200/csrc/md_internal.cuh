@@ -70,7 +70,8 @@ struct DevSys {
   double rc2p[kPairs];             // per-pair cut-off squared (the paper's RCUT(ity,jty)); rc2 is their maximum
   double rc2, rl2, thr2, rin2;     // rin2: build-time split of a list row (pairs with r2 < rin2 first)
   int nc[3], tnc, ncell;           // cells per box (per dim, total) and cells of all boxes
-  int reach;                       // cell side >= (cutoff + skin) / reach: the list build scans (2 reach + 1)^3 cells (1 or 2)
+  int zfine;                       // 1: cubic cells of side >= r_l, 27-cell stencil.  2, 4 (small boxes): cells thinner in z by that
+                                   // factor; the candidates of a column of cells are then a z window around the atom (md_neighbor.cu)
   int cap;                         // neighbour capacity per atom
   int tiles_per_box;               // 32-atom tiles per box
   int kind;
@@ -132,7 +133,7 @@ __device__ __forceinline__ void decide_rebuild(const DevSys &s, bool exceeded, c
   if (go) {
     st->max_neighbors = 0; st->list_entries = 0ull; st->rebuilds += 1;
     for (int a = 0; a < 3; ++a)                        // the cell grid is fixed at md_create; a barostat may have shrunk the box
-      if (!(box_edge(s, a) * s.reach >= s.nc[a] * s.rl)) st->error_flags |= MD_FLAG_BOX;
+      if (!(a == 2 && s.zfine > 1) && !(box_edge(s, a) >= s.nc[a] * s.rl)) st->error_flags |= MD_FLAG_BOX;   // (a z window adapts to the box)
   }
   if (use_cond) { cudaGraphSetConditional(cond, go ? 1u : 0u); if (go) st->graph_body_runs += 1; }
 }

@@ -189,14 +189,15 @@ __device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-
   return v;
 }
 
-// The stencil is (2R+1)^3 cells of side >= r_l / R (R = DevSys::reach: 2, or 1 for very large systems; the paper uses
-// R = 1): with R = 2 a build tests 15.6 cell volumes of candidates instead of 27.
-// PERCELL (every nc >= 2R+3): two atoms of cells within reach WITHOUT crossing the box boundary are closer than
-// (R+1) L/nc <= 0.43 L per axis, and two atoms of cells within reach ACROSS the boundary differ by more than 0.57 L, so
+// The stencil is 3 x 3 columns of cells (cell side >= r_l in x and y), each column ONE contiguous run of slots:
+// ZWIN = false: cubic cells, three cells of z per column; ZWIN = true (small boxes, DevSys::zfine > 1): thinner cells in z
+// and per atom and column the z window that r_l can reach.
+// PERCELL (every edge >= 5 r_l): two atoms of neighbouring cells WITHOUT crossing the box boundary are closer than
+// 0.4 L per axis, and two atoms of cells that are neighbours ACROSS the boundary differ by more than 0.6 L, so
 // the branch of the canonical minimum image is decided by the pair of cells: the shift (0, -L or +L) and its image
 // code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
 // (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
-template <bool PERCELL, int R>
+template <bool PERCELL, bool ZWIN>
 __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
@@ -211,7 +212,8 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   const int cy = cell_coord(pi.y, s.nc[1] / L[1], s.nc[1]);
   const int cz = cell_coord(pi.z, s.nc[2] / L[2], s.nc[2]);
   const int ncx = s.nc[0], ncy = s.nc[1], ncz = s.nc[2];
-  const int zlo = max(cz - R, 0), zhi = min(cz + R, ncz - 1);
+  constexpr int R = 1;
+  const double ax = L[0] / ncx, ay = L[1] / ncy, az = L[2] / ncz;
   int n_all = 0;
   // pairs inside r_in (= r_c) now go to the front of the row (k = 0, 1, ...), skin pairs to the back (k = cap-1, cap-2, ...):
   // the two passes run the full pair evaluation only over the front part (md_force.cu)
@@ -293,19 +295,33 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     if (jy < 0) { jy += ncy; sy = -L[1]; ky = 2; } else if (jy >= ncy) { jy -= ncy; sy = L[1]; ky = 1; }
     const int col = box * s.tnc + (jx * ncy + jy) * ncz;
     const unsigned kxy = kx | (ky << 2);
+    int klo = cz - R, khi = cz + R;
+    if constexpr (ZWIN) {
+      // the z window of this column: every atom of it is at least (gx, gy) away laterally (the gaps to the column's faces),
+      // so only z within w = sqrt(r_l^2 - gx^2 - gy^2) of z_i can be inside r_l; the margins cover the rounding of the
+      // binning (an atom may sit 1e-13 outside the cell it was counted in); L >= 3 r_l: the window never meets itself
+      const double gx = fmax(ox > 0 ? (cx + ox) * ax - pi.x : (ox < 0 ? pi.x - (cx + ox + 1) * ax : 0.0), 0.0);
+      const double gy = fmax(oy > 0 ? (cy + oy) * ay - pi.y : (oy < 0 ? pi.y - (cy + oy + 1) * ay : 0.0), 0.0);
+      const double w2 = s.rl2 * (1.0 + 1e-9) - gx * gx - gy * gy;
+      if (!(w2 > 0.0)) return;
+      const double w = sqrt(w2) + 1e-9;
+      klo = (int)floor((pi.z - w) / az); khi = (int)floor((pi.z + w) / az);
+      khi = min(khi, klo + ncz - 1);
+    }
+    const int zlo = max(klo, 0), zhi = min(khi, ncz - 1);
     for (int run = 0; run < 3; ++run) {                                       // one copy of the candidate loop
       int jbeg, jend;
       double sz = 0.0; unsigned kz = 0;
-      if (run == 0) {                                                         // wrapped cells above: 0 .. cz + R - ncz
-        if (part == 2 || cz + R <= ncz - 1) continue;
-        jbeg = s.cell_start[col]; jend = s.cell_start[col + cz + R - ncz + 1]; sz = L[2]; kz = 1;
+      if (run == 0) {                                                         // wrapped cells above: 0 .. khi - ncz
+        if (part == 2 || khi <= ncz - 1) continue;
+        jbeg = s.cell_start[col]; jend = s.cell_start[col + khi - ncz + 1]; sz = L[2]; kz = 1;
       } else if (run == 1) {                                                  // the in-range z cells
         jbeg = s.cell_start[col + zlo]; jend = s.cell_start[col + zhi + 1];
         if (part == 1) jbeg = max(jbeg, i + 1);
         if (part == 2) jend = min(jend, i);
-      } else {                                                                // wrapped cells below: ncz + cz - R .. ncz - 1
-        if (part == 1 || cz - R >= 0) continue;
-        jbeg = s.cell_start[col + ncz + cz - R]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
+      } else {                                                                // wrapped cells below: ncz + klo .. ncz - 1
+        if (part == 1 || klo >= 0) continue;
+        jbeg = s.cell_start[col + ncz + klo]; jend = s.cell_start[col + ncz]; sz = -L[2]; kz = 2;
       }
       range(jbeg, jend, sx, sy, sz, kxy | (kz << 4));
     }
@@ -473,13 +489,13 @@ int launch_rebuild_body(md_system *sys) {
   {
     ProfScope p(sys, MD_K_LIST);
     const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);
-    const int need = 2 * d.reach + 3;     // cells per edge from which the image of a pair is decided by its pair of cells
-    const bool percell = d.nc[0] >= need && d.nc[1] >= need && d.nc[2] >= need;
+    // edges (in units of r_l) from which the image of a pair is decided by its pair of cells
+    const bool percell = d.nc[0] >= 5 && d.nc[1] >= 5 && d.nc[2] >= 5 * d.zfine;
     ++sys->launches;
-    if (d.reach == 2) {
-      if (percell) k_build_list<true, 2><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, 2><<<gl, kForceBlock, 0, st>>>(d);
+    if (d.zfine > 1) {
+      if (percell) k_build_list<true, true><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, true><<<gl, kForceBlock, 0, st>>>(d);
     } else {
-      if (percell) k_build_list<true, 1><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, 1><<<gl, kForceBlock, 0, st>>>(d);
+      if (percell) k_build_list<true, false><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, false><<<gl, kForceBlock, 0, st>>>(d);
     }
   }
   return (int)cudaGetLastError();

@@ -255,11 +255,12 @@ def test_half_list_passes(md, case, half):
     assert np.abs(gf3 - oracle_of(w, positions=g.positions()).compute_forces()[0]).max() <= F_TOL
 
 
+@pytest.mark.parametrize("zfine", [1, 2, 4])
 @pytest.mark.parametrize("case", ["cfg0_perm", "cfg2_small", "cfg3b_small", "cfg4_small", "noncubic", "alloy_tbsma_boxes"])
-def test_cell_reach_two(md, case, monkeypatch):
-    """The list build with cells of half the list cut-off and a 5 x 5 x 5 stencil (MD_CELL_REACH=2, measured slower on
-    B200 and therefore not the default): the same pair sets, forces and trajectory."""
-    monkeypatch.setenv("MD_CELL_REACH", "2")
+def test_cell_grids(md, case, zfine, monkeypatch):
+    """The list build with cubic cells and with cells 2 or 4 times thinner in z and a z window per column (the default
+    depends on the box size): the same pair sets, forces and trajectory."""
+    monkeypatch.setenv("MD_CELL_ZFINE", str(zfine))
     w = CASES[case]()
     o = oracle_of(w)
     g = md.MDSystem(w)
