@@ -715,6 +715,18 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   const int i = box * s.npb + (valid ? local : 0);
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.posf[i];
+  if (!HALF && kick.h[0] != 0.0) {
+    // the epilogue's velocity (and, chained, x_ref) loads come from DRAM at the very end of the block, when nothing is
+    // left to hide them: ask L2 for their lines now (one line per warp and array)
+    const size_t N = (size_t)s.N;
+    if ((threadIdx.x & 15) == 0) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        asm volatile("prefetch.global.L2 [%0];" :: "l"(s.vel + c * N + i));
+        if (ctl.chain) asm volatile("prefetch.global.L2 [%0];" :: "l"(s.xref + c * N + i));
+      }
+    }
+  }
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
