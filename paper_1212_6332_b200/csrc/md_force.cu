@@ -841,30 +841,67 @@ __device__ __forceinline__ SubMap sub_map(const DevSys &s) {
   return m;
 }
 
-// calls body(entry, in_main) for the entries of the row that this sub-lane owns: whole 16-byte groups round-robin, or
-// (SUB >= 16: rows of a few tens of entries would leave most lanes idle) single entries round-robin
+// calls body(entry, gathered neighbour, in_main) for the entries of the row that this sub-lane owns: whole 16-byte groups
+// round-robin, or (SUB >= 16: rows of a few tens of entries would leave most lanes idle) single entries round-robin.
+// Software pipeline: the entries are loaded two turns ahead and the neighbours of the next turn are gathered before the
+// current turn is evaluated, so that a lane waits for memory once per row, not once per pair.
 template <int SUB, class Body>
-__device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, Body body) {
+__device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, const double4 *__restrict__ pos, Body body) {
   if constexpr (SUB >= 16) {
-    const unsigned *m = reinterpret_cast<const unsigned *>(row.main), *l = reinterpret_cast<const unsigned *>(row.last);
-    for (int k = sl; k < row.n_in; k += SUB) body(__ldg(m + nbr_entry(k)), true);
-    for (int k = sl; k < row.n_out; k += SUB) body(__ldg(l + 3 - (int)nbr_entry(k)), false);   // entry cap-1-k: group -(k>>2), component 3-(k&3)
+    auto part = [&](const unsigned *base, int n, bool in_main, auto at) {
+      int k = sl;
+      if (k >= n) return;
+      unsigned e = __ldg(base + at(k));
+      double4 p = gather32(slot_ptr(pos, MD_GIDX(e)));
+      for (;;) {
+        const int kn = k + SUB;
+        unsigned en = 0u;
+        double4 pn = p;
+        if (kn < n) { en = __ldg(base + at(kn)); pn = gather32(slot_ptr(pos, MD_GIDX(en))); }
+        body(e, p, in_main);
+        if (kn >= n) break;
+        e = en; p = pn; k = kn;
+      }
+    };
+    part(reinterpret_cast<const unsigned *>(row.main), row.n_in, true, [](int k) { return (int)nbr_entry(k); });
+    part(reinterpret_cast<const unsigned *>(row.last), row.n_out, false, [](int k) { return 3 - (int)nbr_entry(k); });   // entry cap-1-k
     return;
-  }
-  constexpr int kSub = SUB;
-  for (int g = sl; g * 4 < row.n_in; g += kSub) {
-    const uint4 E = ldg_group(row.main + (size_t)g * 32);
-    const unsigned e[4] = {E.x, E.y, E.z, E.w};
+  } else {
+    // dir = +1: groups from the front (main part), -1: from the end of the row (skin part, entries in reverse inside a group)
+    auto part = [&](const uint4 *base, int n, bool in_main, int dir) {
+      const int ng = (n + 3) >> 2;
+      int g = sl;
+      if (g >= ng) return;
+      const uint4 none = make_uint4(0u, 0u, 0u, 0u);
+      auto order = [&](const uint4 &E, unsigned (&e)[4]) {
+        if (dir > 0) { e[0] = E.x; e[1] = E.y; e[2] = E.z; e[3] = E.w; } else { e[0] = E.w; e[1] = E.z; e[2] = E.y; e[3] = E.x; }
+      };
+      unsigned e[4], en[4];
+      double4 p[4], pn[4];
+      order(ldg_group(base + (ptrdiff_t)dir * g * 32), e);
+      uint4 En = (g + SUB < ng) ? ldg_group(base + (ptrdiff_t)dir * (g + SUB) * 32) : none;
 #pragma unroll
-    for (int c = 0; c < 4; ++c)
-      if (g * 4 + c < row.n_in) body(e[c], true);
-  }
-  for (int g = sl; g * 4 < row.n_out; g += kSub) {
-    const uint4 E = ldg_group(row.last - (size_t)g * 32);
-    const unsigned e[4] = {E.w, E.z, E.y, E.x};
+      for (int c = 0; c < 4; ++c) p[c] = gather32(slot_ptr(pos, MD_GIDX(e[c])));           // slot 0 for the padding of a partly filled group: harmless
+      for (;;) {
+        const int gn = g + SUB;
+        const bool more = gn < ng;
+        order(En, en);
+        En = (gn + SUB < ng) ? ldg_group(base + (ptrdiff_t)dir * (gn + SUB) * 32) : none;
+        if (more) {
 #pragma unroll
-    for (int c = 0; c < 4; ++c)
-      if (g * 4 + c < row.n_out) body(e[c], false);
+          for (int c = 0; c < 4; ++c) pn[c] = gather32(slot_ptr(pos, MD_GIDX(en[c])));
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+          if (g * 4 + c < n) body(e[c], p[c], in_main);
+        if (!more) break;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { e[c] = en[c]; p[c] = pn[c]; }
+        g = gn;
+      }
+    };
+    part(row.main, row.n_in, true, 1);
+    part(row.last, row.n_out, false, -1);
   }
 }
 
@@ -880,8 +917,7 @@ __global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_consta
   const double4 pi = s.pos[m.i];
   const int ti = MULTI ? (int)pi.w : 0;
   double rho = 0.0;
-  walk_sub<SUB>(row, m.sl, [&](unsigned e, bool in_main) {
-    const double4 pj = gather32(s.pos + MD_GIDX(e));
+  walk_sub<SUB>(row, m.sl, s.pos, [&](unsigned e, const double4 &pj, bool in_main) {
     double dx, dy, dz;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
     // main: TB-SMA is switched off continuously beyond r_c, tables need the strict test; skin: only pairs now inside r_c
@@ -914,8 +950,7 @@ __global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant
   const double4 pi = s.posf[m.i];
   const int ti = MULTI ? s.type[m.i] : 0;
   ForceAcc<OBS> acc;
-  walk_sub<SUB>(row, m.sl, [&](unsigned e, bool in_main) {
-    const double4 pj = gather32(s.posf + MD_GIDX(e));
+  walk_sub<SUB>(row, m.sl, s.posf, [&](unsigned e, const double4 &pj, bool in_main) {
     double dx, dy, dz, g, V = 0.0;
     const double r2 = pair_r2<KIND != MD_POT_TBSMA>(pj, pi, e, s, dx, dy, dz);
     const int tp = MULTI ? ti * s.nt + s.type[e & kIdxMask] : 0;
