@@ -294,7 +294,12 @@ __device__ __forceinline__ void embed(const DevSys &s, int ti, double rho, doubl
 // ------------------------------------------------------------------------------------------------
 struct PairD { double dx, dy, dz, r2, w; unsigned e; };
 
-__device__ __forceinline__ uint4 ldg_group(const uint4 *p) { return __ldg(p); }
+// the list is streamed once per pass: it is read past L1 (no allocation), so that L1 keeps the gathered positions
+__device__ __forceinline__ uint4 ldg_group(const uint4 *p) {
+  uint4 v;
+  asm("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
 #define MD_GIDX(e) ((e) & kIdxMask)
 
 // One 256-bit load per gathered neighbour (LDG.E.256, sm_100) instead of two 128-bit loads.
