@@ -206,7 +206,7 @@ int md_set_option(md_system *s, int option, int value);
 
 /* Kernel classes for md_profile_read */
 enum { MD_K_BIN = 0, MD_K_SCAN, MD_K_SORT, MD_K_REORDER, MD_K_LIST, MD_K_DENSITY, MD_K_FORCE, MD_K_INTEGRATE,
-       MD_K_REDUCE, MD_K_COUNT };
+       MD_K_REDUCE, MD_K_FORCE_CHAINED /* force passes that also perform the next step's drift (inside md_step) */, MD_K_COUNT };
 /* Sum of CUDA-event elapsed time (ms) and number of launches of one kernel class since the last
  * md_profile_reset; synchronises.  Needs MD_OPT_PROFILE. */
 int md_profile_read(md_system *s, int kernel_class, long *launches, double *total_ms);

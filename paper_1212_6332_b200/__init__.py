@@ -21,7 +21,7 @@ MD_OK, MD_EINVAL, MD_EBOX, MD_EOVERFLOW, MD_ENONFINITE, MD_ECUDA, MD_ESTATE = 0,
 MD_FLAG_OVERFLOW, MD_FLAG_NONFINITE = 1, 2
 MD_POT_TBSMA, MD_POT_EAM_TABLE = 0, 1
 MD_OPT_STEP_OBSERVABLES, MD_OPT_PROFILE, MD_OPT_FORCE_VARIANT, MD_OPT_GRAPH, MD_OPT_HALF_LIST = 1, 2, 3, 4, 5
-KERNEL_CLASSES = ("bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce")
+KERNEL_CLASSES = ("bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce", "force_chained")
 
 _D = C.POINTER(C.c_double)
 _I = C.POINTER(C.c_int)

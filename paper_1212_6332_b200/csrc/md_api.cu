@@ -491,7 +491,7 @@ const char *md_strerror(int e) {
 const char *md_version(void) { return "paper_1212_6332_b200 0.1 (sm_100a)"; }
 
 const char *md_kernel_name(int c) {
-  static const char *names[MD_K_COUNT] = {"bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce"};
+  static const char *names[MD_K_COUNT] = {"bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce", "force_chained"};
   return (c >= 0 && c < MD_K_COUNT) ? names[c] : "?";
 }
 

@@ -1159,7 +1159,7 @@ int launch_force(md_system *sys, bool observables, double half_dt, const StepCtl
   const StepCtl ctl = ctlp ? *ctlp : make_ctl(sys, 0.0, none, false, false);
   const int grid = force_blocks(sys);
   {
-    ProfScope p(sys, MD_K_FORCE);
+    ProfScope p(sys, ctl.chain ? MD_K_FORCE_CHAINED : MD_K_FORCE);
     if (sys->d.kind == MD_POT_TBSMA) {
       if (sys->d.tb.fold) launch_force_k<MD_POT_TBSMA, true>(sys, grid, observables, kp, ctl);
       else launch_force_k<MD_POT_TBSMA, false>(sys, grid, observables, kp, ctl);
