@@ -190,6 +190,9 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                           of every step is the body of a conditional node, the force pass of a step also performs
  *                           the next step's first half-kick, drift and displacement check, and the last block of that
  *                           kernel takes the rebuild decision (2 kernel launches per step when no rebuild is due);
+ *                           up to 4,096 atoms (where a conditional node costs more than the two passes) all steps of
+ *                           a graph share ONE loop node that is entered only when a rebuild is due, and the passes
+ *                           are guarded instead (they return at once while a rebuild is pending);
  *                           0: the same kernels as plain launches (every kernel of the rebuild chain is launched and
  *                           returns at once unless a rebuild is due).  MD_OPT_PROFILE implies plain launches.
  *  MD_OPT_HALF_LIST         Newton's third law (the paper's CPU code uses it, its GPU kernels do not).  Bit 0:

@@ -449,8 +449,9 @@ __device__ __forceinline__ void density_term_n(const DevSys &s, const LoopConsts
 }
 
 template <int KIND, bool MULTI, bool FOLD, bool DYN, bool HALF = false>
-__global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s) {
+__global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(const __grid_constant__ DevSys s, const int guard) {
   __shared__ double tab_sm[kExpTabLen];
+  const bool go = step_guard(s, guard);
   // the atom's own loads are issued BEFORE the table staging and its barrier, so that their latency overlaps it
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
@@ -458,6 +459,7 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
   const int i = box * s.npb + (valid ? local : 0);
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.pos[i];
+  if (!go) return;
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
@@ -526,9 +528,9 @@ __global__ void __launch_bounds__(kForceBlock, kDensityMinBlocks) k_density(cons
 
 // Second kernel of a half density pass: rho_i = owned part + received part; F(rho_i), F'(rho_i)
 template <int KIND>
-__global__ void __launch_bounds__(256) k_embed(const __grid_constant__ DevSys s) {
+__global__ void __launch_bounds__(256) k_embed(const __grid_constant__ DevSys s, const int guard) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= s.N) return;
+  if (i >= s.N || !step_guard(s, guard)) return;
   const double4 pi = s.pos[i];
   const double rho = s.rho[i] + fix_take(s.rho_fix + i);
   double F, Fp;
@@ -687,7 +689,7 @@ __device__ __forceinline__ void force_finish(const DevSys &s, const KickParams &
     }
     block_partials<0, 7>(s, v, sm);
   }
-  if (ctl.chain) finish_displacement(s, ctl, d2, smd);
+  if (ctl.chain || ctl.guard >= 0) finish_displacement(s, ctl, d2, smd);
 }
 
 // Half pass, first kernel: the owned part of the force (and of sum V) goes to frc / eatom as it is, the virial partials
@@ -714,12 +716,14 @@ __global__ void __launch_bounds__(kForceBlock, kForceMinBlocks) k_force(const __
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
   __shared__ unsigned long long smd[kForceBlock / 32];
+  const bool go = step_guard(s, ctl.guard);
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
   const int i = box * s.npb + (valid ? local : 0);
   const AtomRow row = atom_row(s, box, local, i, valid);
   const double4 pi = s.posf[i];
+  if (!go) return;
   if (!HALF && kick.h[0] != 0.0) {
     // the epilogue's velocity (and, chained, x_ref) loads come from DRAM at the very end of the block, when nothing is
     // left to hide them: ask L2 for their lines now (one line per warp and array)
@@ -803,6 +807,7 @@ template <bool OBS>
 __global__ void __launch_bounds__(kForceBlock) k_force_half_finish(const __grid_constant__ DevSys s, const KickParams kick, const StepCtl ctl) {
   __shared__ double sm[kForceBlock / 32][8];
   __shared__ unsigned long long smd[kForceBlock / 32];
+  if (!step_guard(s, ctl.guard)) return;
   const int bpb = (s.npb + kForceBlock - 1) / kForceBlock;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * kForceBlock + threadIdx.x;
   const bool valid = local < s.npb;
@@ -821,7 +826,7 @@ __global__ void __launch_bounds__(kForceBlock) k_force_half_finish(const __grid_
     double v[7] = {e_i, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     block_partials<0, 1>(s, v, sm);
   }
-  if (ctl.chain) finish_displacement(s, ctl, d2, smd);
+  if (ctl.chain || ctl.guard >= 0) finish_displacement(s, ctl, d2, smd);
 }
 
 
@@ -911,9 +916,10 @@ __device__ __forceinline__ void walk_sub(const AtomRow &row, int sl, const doubl
 }
 
 template <int KIND, bool MULTI, bool FOLD, int SUB>
-__global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_constant__ DevSys s) {
+__global__ void __launch_bounds__(kForceBlock) k_density_sub(const __grid_constant__ DevSys s, const int guard) {
   constexpr int kSub = SUB;
   __shared__ double tab_sm[kExpTabLen];
+  if (!step_guard(s, guard)) return;
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
@@ -947,6 +953,7 @@ __global__ void __launch_bounds__(kForceBlock) k_force_sub(const __grid_constant
   __shared__ double tab_sm[kExpTabLen];
   __shared__ double sm[kForceBlock / 32][8];
   __shared__ unsigned long long smd[kForceBlock / 32];
+  if (!step_guard(s, ctl.guard)) return;
   unsigned tab = 0;
   LoopConsts lc = {};
   if (KIND == MD_POT_TBSMA) { tab = stage_exp_table(s, tab_sm); lc = load_loop_consts(tab); }
@@ -1061,41 +1068,41 @@ int force_blocks(const md_system *sys) {
 }
 
 template <int KIND, bool FOLD, int SUB>
-static void launch_density_sub(md_system *sys, int grid) {
-  if (sys->d.nt > 1) k_density_sub<KIND, true, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-  else k_density_sub<KIND, false, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+static void launch_density_sub(md_system *sys, int grid, int guard) {
+  if (sys->d.nt > 1) k_density_sub<KIND, true, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
+  else k_density_sub<KIND, false, FOLD, SUB><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
 }
 
 template <int KIND, bool FOLD>
-static void launch_density_k(md_system *sys, int grid) {
+static void launch_density_k(md_system *sys, int grid, int guard) {
   ++sys->launches;
   switch (sub_lanes(sys)) {
-    case 32: launch_density_sub<KIND, FOLD, 32>(sys, grid); return;
-    case 8: launch_density_sub<KIND, FOLD, 8>(sys, grid); return;
-    case 4: launch_density_sub<KIND, FOLD, 4>(sys, grid); return;
+    case 32: launch_density_sub<KIND, FOLD, 32>(sys, grid, guard); return;
+    case 8: launch_density_sub<KIND, FOLD, 8>(sys, grid, guard); return;
+    case 4: launch_density_sub<KIND, FOLD, 4>(sys, grid, guard); return;
   }
   if (sys->d.half & 1) {
-    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    else k_density<KIND, false, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    ++sys->launches, k_embed<KIND><<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d);
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
+    else k_density<KIND, false, FOLD, false, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
+    ++sys->launches, k_embed<KIND><<<(sys->d.N + 255) / 256, 256, 0, sys->stream>>>(sys->d, guard);
     return;
   }
   if (sys->d.dyn_box) {
-    if (sys->d.nt > 1) k_density<KIND, true, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    else k_density<KIND, false, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
+    else k_density<KIND, false, FOLD, true><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
   } else {
-    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
-    else k_density<KIND, false, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d);
+    if (sys->d.nt > 1) k_density<KIND, true, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
+    else k_density<KIND, false, FOLD, false><<<grid, kForceBlock, 0, sys->stream>>>(sys->d, guard);
   }
 }
 
-int launch_density(md_system *sys) {
+int launch_density(md_system *sys, int guard) {
   ProfScope p(sys, MD_K_DENSITY);
   const int grid = force_blocks(sys);
   if (sys->d.kind == MD_POT_TBSMA) {
-    if (sys->d.tb.fold) launch_density_k<MD_POT_TBSMA, true>(sys, grid);
-    else launch_density_k<MD_POT_TBSMA, false>(sys, grid);
-  } else launch_density_k<MD_POT_EAM_TABLE, true>(sys, grid);
+    if (sys->d.tb.fold) launch_density_k<MD_POT_TBSMA, true>(sys, grid, guard);
+    else launch_density_k<MD_POT_TBSMA, false>(sys, grid, guard);
+  } else launch_density_k<MD_POT_EAM_TABLE, true>(sys, grid, guard);
   return (int)cudaGetLastError();
 }
 

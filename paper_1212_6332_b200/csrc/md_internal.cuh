@@ -34,6 +34,9 @@ struct DevState {
   double mu, pressure;             // last barostat step
   unsigned long long graph_body_runs; // rebuild bodies that ran inside a CUDA-graph step (for the launch count)
   unsigned long long step_word;    // running drift / chained force kernel: blocks arrived (low half) | blocks with an atom beyond skin/2 (high half)
+  int k_done;                      // loop graphs (md_api.cu): steps of the current graph launch that are complete
+  int iters_this_launch;           // ... and iterations of its WHILE node (bounded: a loop that makes no progress ends with MD_FLAG_LOOP)
+  unsigned long long loop_iters;   // loop graphs: iterations of their WHILE nodes so far (for the launch count)
 };
 
 struct TbsmaParams {               // per type pair, pre-combined on the host
@@ -109,7 +112,11 @@ struct DevSys {
 
 // What the kernel that ends a drift needs for the rebuild decision (taken by its last block, decide_rebuild below):
 // chain != 0 (force pass only): the epilogue also does the NEXT step's first half-kick, drift and displacement check.
-struct StepCtl { double dt; unsigned long long thr2_bits; cudaGraphConditionalHandle cond; int use_cond; int chain; };
+// guard (loop graphs, md_api.cu): >= 0: this kernel belongs to step `guard` of a graph whose steps all sit in the body of
+// ONE loop: it runs only if no rebuild is pending and exactly `guard` steps are complete (step_guard below), and the force
+// pass that completes the step says so; kGuardReset (the drift at the head of such a graph): zero steps are complete.
+struct StepCtl { double dt; unsigned long long thr2_bits; cudaGraphConditionalHandle cond; int use_cond; int chain; int guard; };
+constexpr int kGuardNone = -1, kGuardReset = -2;
 
 constexpr double kFixScale = 8796093022208.0, kFixInv = 1.0 / 8796093022208.0;   // 2^43: one unit = 1.1e-13 (eV/A, eV, density), range +-1.0e6
 
@@ -161,9 +168,18 @@ __device__ __forceinline__ void finish_displacement(const DevSys &s, const StepC
     const unsigned long long w = atomicAdd(&st->step_word, inc) + inc;
     if ((unsigned)(w & 0xffffffffull) == gridDim.x) {
       st->step_word = 0ull;                              // for the next kernel that ends a drift
-      decide_rebuild(s, (w >> 32) != 0ull, c.cond, c.use_cond);
+      if (c.chain || c.guard == kGuardReset || c.guard == kGuardNone) decide_rebuild(s, (w >> 32) != 0ull, c.cond, c.use_cond);
+      if (c.guard >= 0) st->k_done = c.guard + 1;        // (a step's last force pass without a drift only reports the step complete)
+      if (c.guard == kGuardReset) { st->k_done = 0; st->iters_this_launch = 0; }
     }
   }
+}
+
+// Loop graphs: does this kernel of step `guard` run?  Every block asks (one L2 read, issued before the block's own loads).
+__device__ __forceinline__ bool step_guard(const DevSys &s, int guard) {
+  if (guard < 0) return true;
+  const volatile DevState *st = s.st;
+  return st->do_rebuild == 0 && st->k_done == guard;
 }
 
 struct ProfClass { std::vector<cudaEvent_t> ev; size_t used = 0; long dropped = 0; };
@@ -180,7 +196,9 @@ struct md_system {
   bool have_list, forces_valid, observables_valid;
   bool opt_step_obs, opt_profile, opt_graph;
   // one velocity-Verlet step as a CUDA graph: kick+drift, decision, IF(rebuild body), density, force (md_api.cu)
-  struct StepGraph { cudaGraph_t graph; cudaGraphExec_t exec; double dt; bool obs; int nsteps, kernels; } sg[2];   // [0]: kStepUnroll steps, [1]: the remainder
+  // [0]: kStepUnroll steps, [1]: the remainder.  loop: the steps are the body of ONE while node (small systems); kernels:
+  // launches per replay (loop: with one iteration); iter_kernels: launches of every further iteration
+  struct StepGraph { cudaGraph_t graph; cudaGraphExec_t exec; double dt; bool obs, loop; int nsteps, kernels, iter_kernels; } sg[2];
   int body_kernels;
   int graph_error;                 // cudaError_t of a failed step-graph build (0: none); md_step then uses plain launches
   bool last_step_graph;            // the last md_step replayed the graph
@@ -220,6 +238,8 @@ constexpr int kSubMaxAtoms = 24576;                // at or below this many atom
 constexpr int kSub32MaxAtoms = 4096;               // ... and 32 lanes per atom at or below this many
 constexpr int kSub32Limit = 32768;                 // largest system the 32-lane variant may be forced on (sizes the block partials)
 constexpr int kStepUnroll = 8;                     // time steps per CUDA graph of md_step (md_api.cu)
+constexpr int kLoopGraphMaxAtoms = 4096;           // up to this many atoms the steps of a graph share ONE loop node instead of an IF node each
+                                                   // (measured: 864 atoms 21.9 -> 17.5 us/step; 16,384 and 65,536 atoms: no gain; rebuilds every other step: a loss)
 int sub_lanes(const md_system *s);                 // lanes per atom of the two passes: 1, 2, 4, 8 or 32
 int force_blocks(const md_system *s);              // grid of the two passes (and number of block partials)
 inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block; }
@@ -227,9 +247,12 @@ inline int blocks_per_box(int npb, int block) { return (npb + block - 1) / block
 // launchers (each enqueues on s->stream; returns cudaError_t of the launch)
 int launch_rebuild_chain(md_system *s);                       // decision + body, conditional on DevState (force_rebuild / maxd2)
 int launch_decide(md_system *s, cudaGraphConditionalHandle cond, bool use_cond);
-StepCtl make_ctl(const md_system *s, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain);
+StepCtl make_ctl(const md_system *s, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain, int guard = kGuardNone);
 int launch_rebuild_body(md_system *s);
-int launch_density(md_system *s);
+int launch_density(md_system *s, int guard = kGuardNone);
+int launch_loop_head(md_system *s);                                            // loop graphs: one-thread kernels around the steps
+int launch_loop_tail(md_system *s, cudaGraphConditionalHandle loop_cond, int nsteps);
+int launch_rebuild_done(md_system *s);
 int half_mask(const md_system *s);                            // passes that run as half passes now (0 unless one thread per atom, static box)
 int launch_prepare_tables(md_system *s);                      // md_create, MD_POT_EAM_TABLE: per-interval coefficients
 int launch_force(md_system *s, bool observables, double half_dt, const StepCtl *ctl = nullptr); // half_dt = dt/2 (0: no velocity update); ctl->chain: + next drift

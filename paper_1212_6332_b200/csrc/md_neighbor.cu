@@ -444,11 +444,38 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   }
 }
 
-StepCtl make_ctl(const md_system *sys, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain) {
+StepCtl make_ctl(const md_system *sys, double dt, cudaGraphConditionalHandle cond, bool use_cond, bool chain, int guard) {
   StepCtl c;
   c.dt = dt; c.thr2_bits = (unsigned long long)__builtin_bit_cast(long long, sys->d.thr2);
-  c.cond = cond; c.use_cond = use_cond ? 1 : 0; c.chain = chain ? 1 : 0;
+  c.cond = cond; c.use_cond = use_cond ? 1 : 0; c.chain = chain ? 1 : 0; c.guard = guard;
   return c;
+}
+
+// ---- loop graphs (md_api.cu): the one-thread kernels around the steps of a WHILE body -----------------------------------
+__global__ void k_loop_head(const __grid_constant__ DevSys s) {
+  DevState *st = s.st;
+  st->loop_iters += 1;
+  st->iters_this_launch += 1;
+}
+__global__ void k_rebuild_done(const __grid_constant__ DevSys s) { s.st->do_rebuild = 0; }      // last kernel of the rebuild chain in a loop graph
+__global__ void k_loop_tail(const __grid_constant__ DevSys s, cudaGraphConditionalHandle loop_cond, int nsteps) {
+  // every iteration completes at least one step (a pending rebuild is done first), so nsteps iterations always suffice
+  DevState *st = s.st;
+  const bool stuck = st->k_done < nsteps && st->iters_this_launch > nsteps + 1;
+  if (stuck) st->error_flags |= 1 << 29;
+  cudaGraphSetConditional(loop_cond, (st->k_done < nsteps && !stuck) ? 1u : 0u);
+}
+int launch_loop_head(md_system *sys) {
+  ++sys->launches, k_loop_head<<<1, 1, 0, sys->stream>>>(sys->d);
+  return (int)cudaGetLastError();
+}
+int launch_rebuild_done(md_system *sys) {
+  ++sys->launches, k_rebuild_done<<<1, 1, 0, sys->stream>>>(sys->d);
+  return (int)cudaGetLastError();
+}
+int launch_loop_tail(md_system *sys, cudaGraphConditionalHandle loop_cond, int nsteps) {
+  ++sys->launches, k_loop_tail<<<1, 1, 0, sys->stream>>>(sys->d, loop_cond, nsteps);
+  return (int)cudaGetLastError();
 }
 
 int launch_decide(md_system *sys, cudaGraphConditionalHandle cond, bool use_cond) {
