@@ -49,6 +49,7 @@ def lib():
         _lib.oracle_min_image.argtypes = [_D, _D, _D, _D, _D]
         _lib.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _lib.oracle_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        _lib.oracle_set_integrator.argtypes = [C.c_void_p, C.c_int]
         _lib.oracle_set_barostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
         _lib.oracle_get_box.argtypes = [C.c_void_p, _D]
         _lib.oracle_get_pressure.argtypes = [C.c_void_p, _D]
@@ -153,6 +154,10 @@ class Oracle:
 
     def step(self, n: int, dt: float):
         self._check(lib().oracle_step(self._h, int(n), float(dt)))
+
+    def set_integrator(self, kind: int):
+        """0: velocity-Verlet (default); 1: five-value Gear predictor-corrector."""
+        self._check(lib().oracle_set_integrator(self._h, int(kind)))
 
     def set_thermostat(self, T_e: float, tau: float):
         """eq.(4): electron-bath thermostat (K, fs); tau <= 0 switches it off."""

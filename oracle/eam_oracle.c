@@ -40,6 +40,8 @@ struct oracle_system {
   int stride, *ncount, *nlist, have_list, forces_valid;
   double *rho, *fp, *eemb, *eatom, *wat; /* wat: per-atom virial [N][6] */
   double *virial;                        /* [nb][6] */
+  int integrator, gear_ready;            /* 0: velocity-Verlet; 1: five-value Gear predictor-corrector (its derivatives below) */
+  double *ga, *gj, *gs;                  /* [N][3] acceleration, third and fourth time derivative of x */
   oracle_stats st;
 };
 
@@ -222,7 +224,7 @@ int oracle_destroy(oracle_system *s) {
   free(s->f_val); free(s->f_der); free(s->phi_val); free(s->phi_der); free(s->F_val); free(s->F_der);
   free(s->rc_p); free(s->rc2_p); free(s->ron_p);
   free(s->ncount); free(s->nlist); free(s->rho); free(s->fp); free(s->eemb); free(s->eatom); free(s->wat);
-  free(s->virial); free(s);
+  free(s->virial); free(s->ga); free(s->gj); free(s->gs); free(s);
   return ORACLE_OK;
 }
 
@@ -389,7 +391,7 @@ int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, doub
  * atom at rest.  Each half-kick of the velocity-Verlet step uses the damping of the velocity it starts from. */
 #define KB_EV 8.617333262e-5
 int oracle_set_thermostat(oracle_system *s, double T_e, double tau) {
-  if (!s || !(T_e >= 0.0)) return ORACLE_EINVAL;
+  if (!s || !(T_e >= 0.0) || (tau > 0.0 && s->integrator == 1)) return ORACLE_EINVAL;
   s->thermo_Te = T_e; s->thermo_tau = tau;
   return ORACLE_OK;
 }
@@ -400,7 +402,7 @@ int oracle_set_thermostat(oracle_system *s, double T_e, double tau) {
  * the force evaluation of this step, V = Lx Ly Lz; pressures in eV/A^3, tau_p in fs eV/A^3 (it absorbs the
  * compressibility); x_ref is NOT scaled, so the skin/2 rule also sees the displacement that the scaling causes. */
 int oracle_set_barostat(oracle_system *s, double P0, double tau_p) {
-  if (!s || (tau_p > 0.0 && s->nb != 1)) return ORACLE_EINVAL;
+  if (!s || (tau_p > 0.0 && (s->nb != 1 || s->integrator == 1))) return ORACLE_EINVAL;
   s->baro_P0 = P0; s->baro_tau = tau_p;
   return ORACLE_OK;
 }
@@ -435,6 +437,101 @@ static void half_kick(oracle_system *s, int i, double dt) {
   for (int a = 0; a < 3; ++a) v[a] = v[a] + h * f[a] - (0.5 * dt * g) * v[a];
 }
 
+/* Predictor-corrector integration (sec. 3.3: "A predictor-corrector scheme is used for the stepwise
+ * integration [1] ... Each thread predicts the position and the velocity of one atom"; the velocities
+ * are corrected after the force calculation).  The paper states neither the order nor the coefficients (DESIGN.md
+ * reading G1): taken here as the five-value Gear scheme for m x'' = f(x) in the form of Allen & Tildesley, "Computer
+ * Simulation of Liquids", sec. 3.2 / appendix E: the state is x and its first four time derivatives (v, a, j, s);
+ *   predictor (Taylor):  x_p = x + dt v + dt^2/2 a + dt^3/6 j + dt^4/24 s,   v_p = v + dt a + dt^2/2 j + dt^3/6 s,
+ *                        a_p = a + dt j + dt^2/2 s,   j_p = j + dt s,   s_p = s;
+ *   skin/2 rule on x_p (readings A10, A11), forces at x_p;
+ *   corrector:  D = dt^2/2 (f(x_p)/m - a_p);  x = x_p + c0 D,  v = v_p + c1 D/dt,  a = a_p + c2 D 2/dt^2,
+ *               j = j_p + c3 D 6/dt^3,  s = s_p + c4 D 24/dt^4,   (c0 .. c4) = (19/120, 3/4, 1, 1/2, 1/12).
+ * Start-up: below.  No thermostat, no barostat (velocity-Verlet only). */
+int oracle_set_integrator(oracle_system *s, int kind) {
+  if (!s || (kind != 0 && kind != 1)) return ORACLE_EINVAL;
+  if (kind == 1 && (s->thermo_tau > 0.0 || s->baro_tau > 0.0)) return ORACLE_EINVAL;
+  if (kind == 1 && !s->ga) {
+    s->ga = (double *)calloc(3 * (size_t)s->N, sizeof(double));
+    s->gj = (double *)calloc(3 * (size_t)s->N, sizeof(double));
+    s->gs = (double *)calloc(3 * (size_t)s->N, sizeof(double));
+    if (!s->ga || !s->gj || !s->gs) return ORACLE_EINVAL;
+  }
+  s->integrator = kind; s->gear_ready = 0;
+  return ORACLE_OK;
+}
+
+static int gear_steps(oracle_system *s, int n, double dt) {
+  static const double c0 = 19.0 / 120.0, c1 = 3.0 / 4.0, c2 = 1.0, c3 = 1.0 / 2.0, c4 = 1.0 / 12.0;
+  int rc;
+  const int N = s->N;
+  const double thr = (0.5 * s->skin) * (0.5 * s->skin);
+  const double h1 = dt, h2 = dt * dt / 2.0, h3 = dt * dt * dt / 6.0, h4 = dt * dt * dt * dt / 24.0;
+  if (!s->gear_ready) {
+    /* start-up: a = f(x)/m, and j, s by central differences of a along the Taylor path x(+-tau) = x +- tau v + tau^2/2 a,
+     * tau = dt/10 (with j = s = 0 the first predicted velocity is off by dt^2/2 j and the scheme stays second order) */
+    const double tau = 0.1 * dt;
+    double *x0 = (double *)malloc(3 * (size_t)N * sizeof(double));
+    if (!x0) return ORACLE_EINVAL;
+    memcpy(x0, s->x, 3 * (size_t)N * sizeof(double));
+    if ((rc = forces_internal(s)) != ORACLE_OK) { free(x0); return rc; }
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) s->ga[3 * i + a] = s->f[3 * i + a] / s->m[s->type[i]];
+    for (int k = 0; k < 3 * N; ++k) s->x[k] = x0[k] + tau * s->v[k] + 0.5 * tau * tau * s->ga[k];
+    if ((rc = forces_internal(s)) != ORACLE_OK) { free(x0); return rc; }
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) s->gj[3 * i + a] = s->f[3 * i + a] / s->m[s->type[i]];          /* a(+tau), for now */
+    for (int k = 0; k < 3 * N; ++k) s->x[k] = x0[k] - tau * s->v[k] + 0.5 * tau * tau * s->ga[k];
+    if ((rc = forces_internal(s)) != ORACLE_OK) { free(x0); return rc; }
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) {
+        const int k = 3 * i + a;
+        const double ap = s->gj[k], am = s->f[k] / s->m[s->type[i]];
+        s->gj[k] = (ap - am) / (2.0 * tau);
+        s->gs[k] = ((ap - s->ga[k]) + (am - s->ga[k])) / (tau * tau);
+      }
+    memcpy(s->x, x0, 3 * (size_t)N * sizeof(double));
+    free(x0);
+    s->gear_ready = 1;
+  }
+  for (int step = 0; step < n; ++step) {
+    double maxd2 = 0.0;
+    for (int i = 0; i < N; ++i) {
+      double d2 = 0.0;
+      for (int a = 0; a < 3; ++a) {
+        const int k = 3 * i + a;
+        const double x = s->x[k], v = s->v[k], ac = s->ga[k], j = s->gj[k], q = s->gs[k];
+        s->x[k] = x + h1 * v + h2 * ac + h3 * j + h4 * q;
+        s->v[k] = v + h1 * ac + h2 * j + h3 * q;
+        s->ga[k] = ac + h1 * j + h2 * q;
+        s->gj[k] = j + h1 * q;
+        const double u = s->x[k] - s->xref[k];
+        d2 += u * u;
+      }
+      if (d2 > maxd2) maxd2 = d2;
+      if (!(d2 == d2)) maxd2 = INFINITY;
+    }
+    s->st.last_max_disp2 = maxd2;
+    if (maxd2 > thr && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
+    if ((rc = forces_internal(s)) != ORACLE_OK) return rc;
+    for (int i = 0; i < N; ++i) {
+      const double m = s->m[s->type[i]];
+      for (int a = 0; a < 3; ++a) {
+        const int k = 3 * i + a;
+        const double D = h2 * (s->f[k] / m - s->ga[k]);
+        s->x[k] += c0 * D;
+        s->v[k] += c1 * D / h1;
+        s->ga[k] += c2 * D / h2;
+        s->gj[k] += c3 * D / h3;
+        s->gs[k] += c4 * D / h4;
+      }
+    }
+    s->forces_valid = 0;       /* f belongs to the predicted coordinates: a query evaluates the corrected ones */
+    s->st.steps += 1;
+  }
+  return ORACLE_OK;
+}
+
 /* Velocity-Verlet (BASELINE.json north_star) with the skin/2 rule (readings A10, A11):
  *   v += (dt/2)(f/m + a_fric(v)); x += dt v; if max_i |x_i - x_ref,i|^2 > (skin/2)^2: rebuild;
  *   f <- force(x); v += (dt/2)(f/m + a_fric(v)). */
@@ -442,6 +539,7 @@ int oracle_step(oracle_system *s, int n, double dt) {
   int rc;
   if (!s || n < 0) return ORACLE_EINVAL;
   if (!s->have_list && (rc = oracle_build_neighbors(s, 0)) != ORACLE_OK) return rc;
+  if (s->integrator == 1) return gear_steps(s, n, dt);
   if (!s->forces_valid && (rc = forces_internal(s)) != ORACLE_OK) return rc;
   const int N = s->N;
   const double thr = (0.5 * s->skin) * (0.5 * s->skin);
@@ -478,9 +576,9 @@ int oracle_step(oracle_system *s, int n, double dt) {
 int oracle_get_positions(oracle_system *s, double *x) { memcpy(x, s->x, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
 int oracle_get_velocities(oracle_system *s, double *v) { memcpy(v, s->v, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
 int oracle_set_positions(oracle_system *s, const double *x) {
-  memcpy(s->x, x, 3 * (size_t)s->N * sizeof(double)); s->have_list = 0; s->forces_valid = 0; s->f_prescale = 0; return ORACLE_OK;
+  memcpy(s->x, x, 3 * (size_t)s->N * sizeof(double)); s->have_list = 0; s->forces_valid = 0; s->f_prescale = 0; s->gear_ready = 0; return ORACLE_OK;
 }
-int oracle_set_velocities(oracle_system *s, const double *v) { memcpy(s->v, v, 3 * (size_t)s->N * sizeof(double)); return ORACLE_OK; }
+int oracle_set_velocities(oracle_system *s, const double *v) { memcpy(s->v, v, 3 * (size_t)s->N * sizeof(double)); s->gear_ready = 0; return ORACLE_OK; }
 
 int oracle_get_neighbors(oracle_system *s, int *count, int *list, int stride) {
   if (!s->have_list) return ORACLE_ESTATE;

@@ -62,6 +62,7 @@ int oracle_set_threads(int n);                           /* OpenMP threads; retu
 int oracle_build_neighbors(oracle_system *s, int mode);
 int oracle_compute_forces(oracle_system *s, double *forces, double *e_atom, double *virial /*[n_boxes][6]*/);
 int oracle_step(oracle_system *s, int n, double dt);
+int oracle_set_integrator(oracle_system *s, int kind);   /* 0: velocity-Verlet (default); 1: five-value Gear predictor-corrector */
 /* eq.(4): electron-bath thermostat at temperature T_e (K) with time constant tau (fs); tau <= 0: off */
 int oracle_set_thermostat(oracle_system *s, double T_e, double tau);
 /* eq.(5)-(6): Berendsen barostat, P0 in eV/A^3, tau_p in fs eV/A^3; tau_p <= 0: off; one box only */

@@ -780,3 +780,81 @@ def test_oracle_under_address_and_undefined_sanitizers(tmp_path):
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
     assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr and "LeakSanitizer" not in r.stderr
     assert "asan-main ok" in r.stdout
+
+
+# --------------------------------------------------------------------------------------
+# Gear predictor-corrector (reading G1)
+# --------------------------------------------------------------------------------------
+def _smooth_cluster():
+    """Four Cu atoms 2.4-2.9 A apart in the 21.7 A box of config 0: every pair stays inside the taper onset (4.4 A), so
+    the potential is analytic along the trajectory and an integrator shows its formal order."""
+    w = workloads.config(0)
+    x = np.array([[5, 5, 5], [7.5, 5.1, 5.0], [6.2, 7.2, 5.1], [6.3, 5.8, 7.1]], dtype=np.float64)
+    v = np.array([[0.01, 0, 0.005], [-0.01, 0.004, 0], [0, -0.006, 0.003], [0.0, 0.002, -0.008]])
+    return w, dict(positions=x, velocities=v, types=np.zeros(4, np.int32))
+
+
+def _run(w, kw, kind, dt, t_end):
+    o = Oracle(w, **kw)
+    o.set_integrator(kind)
+    o.step(int(round(t_end / dt)), dt)
+    return o
+
+
+def test_gear_order_of_accuracy_and_agreement_with_velocity_verlet():
+    """The five-value Gear scheme with coefficients (19/120, 3/4, 1, 1/2, 1/12) converges with the fifth power of dt on
+    a smooth potential (halving dt divides the error by ~32); a wrong coefficient (19/90 for 19/120, a wrong Pascal
+    entry of the predictor) or a start-up with zero higher derivatives leaves second to fourth order (ratio 4 ... 20).
+    Both integrators converge to the same trajectory."""
+    w, kw = _smooth_cluster()
+    T = 32.0
+    ref = _run(w, kw, 1, 1.0 / 32, T).positions()
+    err = [np.abs(_run(w, kw, 1, dt, T).positions() - ref).max() for dt in (2.0, 1.0, 0.5)]
+    assert err[0] < 5e-6 and 26.0 < err[0] / err[1] < 40.0 and 26.0 < err[1] / err[2] < 40.0
+    vv = [np.abs(_run(w, kw, 0, dt, T).positions() - ref).max() for dt in (1.0, 0.5)]
+    assert 3.5 < vv[0] / vv[1] < 4.5                                   # velocity-Verlet: second order, same limit
+    assert np.abs(_run(w, kw, 0, 1.0 / 64, T).positions() - ref).max() < 2e-8
+
+
+def test_gear_free_flight_momentum_and_energy():
+    w, kw = _smooth_cluster()
+    # atoms out of each other's reach: straight lines
+    far = dict(kw, positions=np.array([[1, 1, 1], [11, 1.5, 2], [2, 12, 3], [12, 11, 13]], dtype=np.float64))
+    o = _run(w, far, 1, 1.0, 40.0)
+    assert np.abs(o.positions() - (far["positions"] + 40.0 * far["velocities"])).max() < 1e-12
+    assert np.abs(o.velocities() - far["velocities"]).max() < 1e-15
+    # crystal at 300 K: total momentum constant, energy conserved far better than by velocity-Verlet at the same dt,
+    # rebuilds as often as velocity-Verlet (the skin/2 rule acts on the predicted positions)
+    w0 = workloads.config(0)
+    m = w0.mass[0]
+    res = {}
+    for kind in (0, 1):
+        o = Oracle(w0)
+        o.set_integrator(kind)
+        e0 = sum(e.sum() for e in o.energies())
+        p0 = m * o.velocities().sum(axis=0)
+        o.step(100, 1.0)
+        res[kind] = abs(sum(e.sum() for e in o.energies()) - e0) / w0.n_atoms
+        assert np.abs(m * o.velocities().sum(axis=0) - p0).max() < 1e-10
+        assert o.stats()["rebuilds"] >= 4 and o.list_covers_cutoff()
+    assert res[1] < 1e-7 and res[1] < 0.05 * res[0]
+    # one step is not the same as velocity-Verlet's (the corrector also moves the positions)
+    a, b = Oracle(w0), Oracle(w0)
+    b.set_integrator(1)
+    a.step(1, 1.0); b.step(1, 1.0)
+    d = np.abs(a.positions() - b.positions()).max()
+    assert 1e-9 < d < 1e-4
+
+
+def test_gear_refuses_thermostat_and_barostat():
+    w0 = workloads.config(0)
+    o = Oracle(w0)
+    o.set_integrator(1)
+    with pytest.raises(OracleError):
+        o.set_thermostat(300.0, 100.0)
+    with pytest.raises(OracleError):
+        o.set_barostat(0.0, 1e4)
+    o.set_integrator(0)
+    o.set_thermostat(300.0, 100.0)
+    with pytest.raises(OracleError):
+        o.set_integrator(1)
