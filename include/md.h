@@ -139,6 +139,16 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
  * decision is taken on the device. */
 int md_step(md_system *s, int n, double dt);
 
+/* Integrator.  MD_INT_VERLET (default): velocity-Verlet as described at md_step.  MD_INT_GEAR5: the paper's
+ * predictor-corrector scheme (sec. 3.3), taken as the five-value Gear scheme (the paper gives
+ * neither order nor coefficients): per step  predict x, v, a, j, s by their Taylor series;  skin/2 rule on the predicted
+ * positions;  f = force(x_p);  D = dt^2/2 (f/m - a_p);  x += 19/120 D, v += 3/4 D/dt, a += D 2/dt^2, j += 1/2 D 6/dt^3,
+ * s += 1/12 D 24/dt^4.  The first step after md_create / md_set_* takes a = f(x)/m and j, s from central differences of
+ * a along x(+-dt/10) (two more force evaluations).  Positions returned are the corrected ones.  No thermostat and no
+ * barostat with MD_INT_GEAR5 (MD_EINVAL either way round); its steps are plain kernel launches. */
+enum { MD_INT_VERLET = 0, MD_INT_GEAR5 = 1 };
+int md_set_integrator(md_system *s, int integrator);
+
 /* Electron-bath thermostat of eq.(4) (Finnis et al.):  m dv/dt = f - (m/tau)((T_i - T_e)/T_i) v  with the
  * per-atom instantaneous temperature T_i = m |v|^2 / (3 k_B).  T_e in K, tau in fs (a time: the printed 1/tau_T stands
  * for m_i/tau_T); tau <= 0 switches it off (default).  Inside md_step each half-kick becomes

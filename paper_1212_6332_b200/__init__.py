@@ -21,6 +21,7 @@ MD_OK, MD_EINVAL, MD_EBOX, MD_EOVERFLOW, MD_ENONFINITE, MD_ECUDA, MD_ESTATE = 0,
 MD_FLAG_OVERFLOW, MD_FLAG_NONFINITE = 1, 2
 MD_POT_TBSMA, MD_POT_EAM_TABLE = 0, 1
 MD_OPT_STEP_OBSERVABLES, MD_OPT_PROFILE, MD_OPT_FORCE_VARIANT, MD_OPT_GRAPH, MD_OPT_HALF_LIST = 1, 2, 3, 4, 5
+MD_INT_VERLET, MD_INT_GEAR5 = 0, 1
 KERNEL_CLASSES = ("bin", "scan", "sort", "reorder", "list", "density", "force", "integrate", "reduce", "force_chained")
 
 _D = C.POINTER(C.c_double)
@@ -79,6 +80,7 @@ def lib() -> C.CDLL:
         L.md_get_energies.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_get_stats.argtypes = [C.c_void_p, C.POINTER(MdStats)]
         L.md_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.md_set_integrator.argtypes = [C.c_void_p, C.c_int]
         L.md_set_thermostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.md_set_barostat.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.md_get_box.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
@@ -269,6 +271,10 @@ class MDSystem:
         st = MdStats()
         check(lib().md_get_stats(self._h, C.byref(st)))
         return {k: getattr(st, k) for k, _ in MdStats._fields_}
+
+    def set_integrator(self, integrator: int):
+        """MD_INT_VERLET (default) or MD_INT_GEAR5, the paper's predictor-corrector scheme."""
+        check(lib().md_set_integrator(self._h, int(integrator)))
 
     def set_thermostat(self, T_e: float, tau: float):
         """eq.(4) electron-bath thermostat (K, fs); tau <= 0 switches it off."""

@@ -119,6 +119,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   t.pos = b.take<double4>(N); t.posf = b.take<double4>(N); t.pos_tmp = b.take<double4>(N); t.pos32 = b.take<float4>(N);
   t.vel = b.take<double>(3 * N); t.vel_tmp = b.take<double>(3 * N);
   t.frc = b.take<double>(3 * N); t.xref = b.take<double>(3 * N);
+  t.gacc = b.take<double>(3 * N); t.gjrk = b.take<double>(3 * N); t.gsnp = b.take<double>(3 * N);
   t.type = b.take<int>(N); t.type_tmp = b.take<int>(N); t.orig = b.take<int>(N); t.orig_tmp = b.take<int>(N);
   t.cell_id = b.take<int>(N); t.perm = b.take<int>(N);
   t.cell_count = b.take<int>((size_t)g.ncell + 1); t.cell_start = b.take<int>((size_t)g.ncell + 1);
@@ -144,7 +145,7 @@ static size_t layout(const md_desc *d, const Geometry &g, void *base, md_system 
   if (sys) {
     DevSys &o = sys->d;
     o.st = t.st; o.pos = t.pos; o.posf = t.posf; o.pos_tmp = t.pos_tmp; o.pos32 = t.pos32; o.vel = t.vel; o.vel_tmp = t.vel_tmp;
-    o.frc = t.frc; o.xref = t.xref; o.type = t.type; o.type_tmp = t.type_tmp; o.orig = t.orig; o.orig_tmp = t.orig_tmp;
+    o.frc = t.frc; o.xref = t.xref; o.gacc = t.gacc; o.gjrk = t.gjrk; o.gsnp = t.gsnp; o.type = t.type; o.type_tmp = t.type_tmp; o.orig = t.orig; o.orig_tmp = t.orig_tmp;
     o.cell_id = t.cell_id; o.perm = t.perm; o.cell_count = t.cell_count; o.cell_start = t.cell_start;
     o.cell_fill = t.cell_fill; o.scan_block = t.scan_block; o.nbr = t.nbr; o.ncount = t.ncount; o.rho = t.rho;
     o.nown = t.nown; o.rho_fix = t.rho_fix; o.frc_fix = t.frc_fix;
@@ -568,7 +569,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   s->stream = (cudaStream_t)d->stream;
   s->cutoff = d->cutoff; s->skin = d->skin;
   s->have_list = s->forces_valid = s->observables_valid = false;
-  s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->opt_half = -1; s->steps = 0; s->launches = 0;
+  s->opt_step_obs = s->opt_profile = false; s->opt_graph = true; s->opt_force_variant = 0; s->opt_half = -1; s->integrator = MD_INT_VERLET; s->gear_ready = false; s->steps = 0; s->launches = 0;
   s->thermo_Te = 0.0; s->thermo_tau = 0.0; s->baro_P0 = 0.0; s->baro_tau = 0.0;
   for (auto &g : s->sg) { g.graph = nullptr; g.exec = nullptr; g.dt = 0.0; g.obs = false; g.loop = false; g.nsteps = 0; g.kernels = 0; g.iter_kernels = 0; }
   s->body_kernels = 0;
@@ -695,15 +696,22 @@ int md_set_option(md_system *s, int option, int value) {
   return MD_EINVAL;
 }
 
+int md_set_integrator(md_system *s, int integrator) {
+  if (!s || (integrator != MD_INT_VERLET && integrator != MD_INT_GEAR5)) return MD_EINVAL;
+  if (integrator == MD_INT_GEAR5 && (s->thermo_tau > 0.0 || s->baro_tau > 0.0)) return MD_EINVAL;
+  if (integrator != s->integrator) { s->integrator = integrator; s->gear_ready = false; s->forces_valid = false; s->observables_valid = false; }
+  return MD_OK;
+}
+
 int md_set_thermostat(md_system *s, double T_e, double tau) {
-  if (!s || !(T_e >= 0.0) || !isfinite(T_e) || !isfinite(tau)) return MD_EINVAL;
+  if (!s || !(T_e >= 0.0) || !isfinite(T_e) || !isfinite(tau) || (tau > 0.0 && s->integrator == MD_INT_GEAR5)) return MD_EINVAL;
   s->thermo_Te = T_e; s->thermo_tau = tau;
   drop_step_graph(s);                                // the half-kick parameters are baked into the graph's nodes
   return MD_OK;
 }
 
 int md_set_barostat(md_system *s, double P0, double tau_p) {
-  if (!s || !isfinite(P0) || !isfinite(tau_p) || (tau_p > 0.0 && s->d.nb != 1)) return MD_EINVAL;
+  if (!s || !isfinite(P0) || !isfinite(tau_p) || (tau_p > 0.0 && (s->d.nb != 1 || s->integrator == MD_INT_GEAR5))) return MD_EINVAL;
   s->baro_P0 = P0; s->baro_tau = tau_p;
   drop_step_graph(s);                                // parameters are baked into the graph's nodes
   if (tau_p > 0.0) s->d.dyn_box = 1;                 // kernels read the box edges from device state from now on
@@ -781,6 +789,22 @@ int md_step(md_system *s, int n, double dt) {
   int rc;
   if (n == 0) return MD_OK;
   if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+  if (s->integrator == MD_INT_GEAR5) {
+    // the paper's predictor-corrector (md_gear.cu): predict + displacement check, conditional rebuild, density, force at the
+    // predicted positions, correct; plain launches
+    if (!s->gear_ready) {
+      if ((rc = forces_sequence(s, false, 0.0)) != MD_OK) return rc;
+      if (launch_gear_start(s, dt) != 0) return MD_ECUDA;
+      s->gear_ready = true;
+    }
+    for (int k = 0; k < n; ++k)
+      if (launch_gear_predict(s, dt) != 0 || launch_rebuild_body(s) != 0 || launch_density(s) != 0 || launch_force(s, s->opt_step_obs, 0.0) != 0 ||
+          launch_gear_correct(s, dt) != 0) return MD_ECUDA;
+    s->last_step_graph = false;
+    s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;   // frc belongs to the predicted positions: queries evaluate the corrected ones
+    s->steps += n;
+    return MD_OK;
+  }
   if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
   const bool baro = s->baro_tau > 0.0;
   const bool obs = s->opt_step_obs || baro;          // the barostat needs the virial of every step
@@ -842,7 +866,7 @@ int md_set_positions(md_system *s, const double *x) {
     src = (const double *)s->stage;
   }
   ++s->launches, k_set_pos<<<grid_for(o.N), 256, 0, s->stream>>>(o, src, s->have_list ? 1 : 0);
-  s->forces_valid = false; s->observables_valid = false; s->frc_keep = false;
+  s->forces_valid = false; s->observables_valid = false; s->frc_keep = false; s->gear_ready = false;
   if (src != x && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;   // the host buffer may be reused
   return check_cuda(cudaGetLastError());
 }
@@ -862,6 +886,7 @@ int md_set_state(md_system *s, const double *x, const double *v) {
     vs = (const double *)((char *)s->stage + bytes); host = true;
   }
   int *flag = o.scan_block;                            // free outside the rebuild chain
+  s->gear_ready = false;
   if (cudaMemsetAsync(flag, 0, sizeof(int), s->stream) != cudaSuccess) return MD_ECUDA;
   ++s->launches, k_set_state<<<grid_for(o.N), 256, 0, s->stream>>>(o, xs, vs, s->have_list ? 1 : 0, flag);
   if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
@@ -904,6 +929,7 @@ int md_set_velocities(md_system *s, const double *v) {
     src = (const double *)s->stage;
   }
   ++s->launches, k_set_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, src);
+  s->gear_ready = false;
   if (src != v && cudaStreamSynchronize(s->stream) != cudaSuccess) return MD_ECUDA;
   return check_cuda(cudaGetLastError());
 }

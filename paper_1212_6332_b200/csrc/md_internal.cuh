@@ -83,6 +83,7 @@ struct DevSys {
   double4 *posf;                   // x,y,z, w = F'(rho): written by the density pass, gathered by the force pass
   float4 *pos32;                   // x,y,z rounded to float at the last re-order: the list build's single-precision filter
   double *vel, *frc, *xref;        // SoA, component c at [c*N + i]
+  double *gacc, *gjrk, *gsnp;      // Gear predictor-corrector (md_gear.cu): second, third and fourth time derivative of x, SoA
   int *type, *orig;                // orig = caller index of the atom in this slot (paper's hGID)
   // re-order scratch
   double4 *pos_tmp; double *vel_tmp; int *type_tmp, *orig_tmp;
@@ -204,6 +205,7 @@ struct md_system {
   bool last_step_graph;            // the last md_step replayed the graph
   bool frc_keep;                   // frc holds the forces of the coordinates BEFORE the barostat scaled them: queries must not replace them
   int opt_force_variant, opt_half;
+  int integrator; bool gear_ready; // MD_INT_*; the derivative arrays of the Gear scheme belong to the current x, v
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
@@ -258,6 +260,10 @@ int launch_prepare_tables(md_system *s);                      // md_create, MD_P
 int launch_force(md_system *s, bool observables, double half_dt, const StepCtl *ctl = nullptr); // half_dt = dt/2 (0: no velocity update); ctl->chain: + next drift
 int launch_kick_drift(md_system *s, double dt, const StepCtl &ctl);
 int launch_ekin(md_system *s);
+int launch_gear_start(md_system *s, double dt);               // md_gear.cu: the paper's predictor-corrector (five-value Gear scheme)
+int launch_gear_predict(md_system *s, double dt);
+int launch_gear_correct(md_system *s, double dt);
+int launch_gear_reorder(md_system *s);
 int launch_barostat(md_system *s, double dt);                 // ekin, mu and box update, scale positions (end of a step)
 int launch_pressure(md_system *s);                            // ekin + eq.(6) into DevState::pressure
 

@@ -513,6 +513,7 @@ int launch_rebuild_body(md_system *sys) {
     ++sys->launches, k_reorder<<<gN, tb, 0, st>>>(d);
     ++sys->launches, k_copyback<<<gN, tb, 0, st>>>(d);
   }
+  if (sys->integrator == MD_INT_GEAR5 && launch_gear_reorder(sys) != 0) return 1;
   {
     ProfScope p(sys, MD_K_LIST);
     const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);

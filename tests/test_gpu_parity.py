@@ -520,6 +520,72 @@ def test_set_get_state(md):
     assert np.array_equal(xt.cpu().numpy(), b.positions())
 
 
+@pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 60), ("cfg1_small", 60), ("cfg2_small", 60), ("cfg3b_small", 40),
+                                         ("cfg4_small", 60), ("alloy_tbsma_boxes", 60), ("alloy4_tables_rcut", 60)])
+def test_gear_predictor_corrector_trajectory(md, case, nsteps):
+    """Row f4, the paper's predictor-corrector integration as the five-value Gear scheme: the
+    same start-up, predictor, skin/2 rule on the predicted positions, and corrector as the oracle."""
+    w = CASES[case]()
+    o = oracle_of(w)
+    g = md.MDSystem(w)
+    o.set_integrator(1)
+    g.set_integrator(md.MD_INT_GEAR5)
+    e0 = sum(x.sum() for x in g.energies())
+    for n in (1, nsteps - 1):                       # (two calls: the derivative arrays carry over)
+        o.step(n, w.dt)
+        g.step(n, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL
+    assert np.abs(g.velocities() - o.velocities()).max() <= 1e-9
+    so, sg = o.stats(), g.stats()
+    assert sg["steps"] == nsteps and sg["error_flags"] == 0 and sg["graph_active"] == 0
+    assert abs(sg["rebuilds"] - so["rebuilds"]) <= 1 and sg["rebuilds"] >= 2
+    oep, oek = o.energies()
+    gep, gek = g.energies()
+    assert abs((gep.sum() + gek.sum()) - (oep.sum() + oek.sum())) <= 1e-10 * abs(oep.sum())
+    if case == "cfg0":
+        assert abs(gep.sum() + gek.sum() - e0) / w.n_atoms < 1e-7          # two orders better than velocity-Verlet at this dt
+    # new velocities restart the scheme (a, j, s are rebuilt from the new state), on both sides alike
+    v = 0.9 * g.velocities()
+    g.set_velocities(v)
+    o.set_velocities(v)
+    g.step(10, w.dt)
+    o.step(10, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL
+    # back to velocity-Verlet
+    g.set_integrator(md.MD_INT_VERLET)
+    o.set_integrator(0)
+    g.step(10, w.dt)
+    o.step(10, w.dt)
+    d = g.positions() - o.positions()
+    d -= np.round(d / w.box) * w.box
+    assert np.abs(d).max() <= X_TOL and g.stats()["error_flags"] == 0
+
+
+def test_gear_refusals_and_determinism(md):
+    w = CASES["cfg3a_small"]()
+    g = md.MDSystem(w)
+    g.set_integrator(md.MD_INT_GEAR5)
+    with pytest.raises(md.MDError):
+        g.set_thermostat(300.0, 100.0)
+    with pytest.raises(md.MDError):
+        g.set_barostat(0.0, 1e4)
+    with pytest.raises(md.MDError):
+        g.set_integrator(7)
+    g.step(30, 1.0)
+    h = md.MDSystem(w)
+    h.set_integrator(md.MD_INT_GEAR5)
+    h.step(30, 1.0)
+    assert np.array_equal(g.positions(), h.positions()) and np.array_equal(g.velocities(), h.velocities())
+    t = md.MDSystem(w)
+    t.set_thermostat(300.0, 100.0)
+    with pytest.raises(md.MDError):
+        t.set_integrator(md.MD_INT_GEAR5)
+
+
 def test_diagnostics_run(md):
     rate, mhz = md.fp64_dfma_rate()
     assert rate > 1e12 and mhz > 500
