@@ -572,9 +572,14 @@ __device__ __forceinline__ void force_term(const DevSys &s, const LoopConsts &lc
     double t;
     const int k = table_index(s.tab, r, t);
     const size_t o = (size_t)tp * (s.tab.nr - 1) + k;
-    const double4 cf = ldg4(s.tab.der_c + 2 * o), cp = ldg4(s.tab.der_c + 2 * o + 1);
-    const double df = fma(t, fma(t, cf.z, cf.y), cf.x);
-    const double dV = fma(t, fma(t, cp.z, cp.y), cp.x);
+    // 48-byte records (fd1, fd2, fd3, pd1, pd2, pd3): always two sectors, and a quarter less of L1 than padded 64-byte ones
+    const double2 *rec = reinterpret_cast<const double2 *>(s.tab.der_c) + 3 * o;
+    double2 a, b, c;
+    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a.x), "=d"(a.y) : "l"(rec));
+    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(b.x), "=d"(b.y) : "l"(rec + 1));
+    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(c.x), "=d"(c.y) : "l"(rec + 2));
+    const double df = fma(t, fma(t, b.x, a.y), a.x);
+    const double dV = fma(t, fma(t, c.y, c.x), b.y);
     g = fma(fp_sum, df, dV) * rinv;
     if (OBS) { const double4 c = ldg4(s.tab.phi_c + o); V = fma(t, fma(t, fma(t, c.w, c.z), c.y), c.x); }
   }
@@ -1027,8 +1032,9 @@ __global__ void k_prepare_tables(const __grid_constant__ DevSys s, double4 *f_c,
   const double ih = s.tab.inv_dr;
   f_c[g] = cf;
   phi_c[g] = cp;
-  der_c[2 * g] = make_double4(cf.y * ih, 2.0 * cf.z * ih, 3.0 * cf.w * ih, 0.0);
-  der_c[2 * g + 1] = make_double4(cp.y * ih, 2.0 * cp.z * ih, 3.0 * cp.w * ih, 0.0);
+  double *rec = reinterpret_cast<double *>(der_c) + 6 * g;
+  rec[0] = cf.y * ih; rec[1] = 2.0 * cf.z * ih; rec[2] = 3.0 * cf.w * ih;
+  rec[3] = cp.y * ih; rec[4] = 2.0 * cp.z * ih; rec[5] = 3.0 * cp.w * ih;
 }
 
 int launch_prepare_tables(md_system *sys) {
