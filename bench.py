@@ -270,6 +270,7 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
 
     # ---- device-resident run: W warm-up steps, then exactly K timed steps ------------------------------
     g.step(W, w.dt)
+    g.prepare_step(K, w.dt)                          # graph instantiation for md_step(K) is set-up, not a time step
     st0 = g.stats()
     sampler = ClockSampler(local_rank)
     barrier()
@@ -350,6 +351,7 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
         hxn, hvn = hx.numpy(), hv.numpy()
         g.get_state(out=(hxn, hvn))
         Ke = min(K, args.e2e_steps) if args.e2e_steps else K
+        g.prepare_step(1, w.dt)
         for _ in range(3):
             g.set_state(hxn, hvn); g.step(1, w.dt); g.get_state(out=(hxn, hvn))
         barrier()

@@ -138,6 +138,10 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
  * the first step if they are stale.  Nothing crosses the host/device boundary inside the call; the rebuild
  * decision is taken on the device. */
 int md_step(md_system *s, int n, double dt);
+/* Optional: build, instantiate and upload the CUDA graphs that md_step(n, dt) will replay, without taking a step (set-up
+ * work of a few milliseconds that md_step otherwise does on the first call with a new (n mod 8, dt)).  No effect with
+ * MD_OPT_GRAPH 0, MD_OPT_PROFILE 1 or MD_INT_GEAR5. */
+int md_prepare_step(md_system *s, int n, double dt);
 
 /* Integrator.  MD_INT_VERLET (default): velocity-Verlet as described at md_step.  MD_INT_GEAR5: the paper's
  * predictor-corrector scheme (sec. 3.3), taken as the five-value Gear scheme (the paper gives

@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
             getattr(L, name).argtypes = [C.c_void_p]
         L.md_compute_forces.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.md_prepare_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
         for name in ("md_get_positions", "md_get_velocities", "md_set_positions", "md_set_velocities"):
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
         for name in ("md_set_state", "md_get_state"):
@@ -217,6 +218,10 @@ class MDSystem:
 
     def step(self, n: int, dt: float):
         check(lib().md_step(self._h, int(n), float(dt)))
+
+    def prepare_step(self, n: int, dt: float):
+        """Build the CUDA graphs step(n, dt) will replay (set-up work, no time step)."""
+        check(lib().md_prepare_step(self._h, int(n), float(dt)))
 
     def positions(self, device_out: bool = False, out=None):
         x = out if out is not None else self._out((self.n_atoms, 3), np.float64, device_out)

@@ -784,6 +784,18 @@ int md_compute_forces(md_system *s, double *forces, double *e_atom, double *viri
   return any_host ? sync_and_flags(s) : MD_OK;
 }
 
+int md_prepare_step(md_system *s, int n, double dt) {
+  if (!s || n < 0 || !isfinite(dt)) return MD_EINVAL;
+  if (n == 0 || !s->opt_graph || s->opt_profile || s->integrator != MD_INT_VERLET) return MD_OK;
+  const bool baro = s->baro_tau > 0.0, obs = s->opt_step_obs || baro;
+  const int unroll = baro ? 1 : kStepUnroll, q = n / unroll, r = n % unroll;
+  if ((q > 0 && build_step_graph(s, s->sg[0], dt, obs, unroll) != MD_OK) || (r > 0 && build_step_graph(s, s->sg[1], dt, obs, r) != MD_OK))
+    return MD_OK;                                      // md_step will run the same kernels as plain launches (md_stats.graph_error says why)
+  if (q > 0) cudaGraphUpload(s->sg[0].exec, s->stream);
+  if (r > 0) cudaGraphUpload(s->sg[1].exec, s->stream);
+  return cudaGetLastError() == cudaSuccess ? MD_OK : MD_ECUDA;
+}
+
 int md_step(md_system *s, int n, double dt) {
   if (!s || n < 0 || !isfinite(dt)) return MD_EINVAL;
   int rc;

@@ -586,6 +586,24 @@ def test_gear_refusals_and_determinism(md):
         t.set_integrator(md.MD_INT_GEAR5)
 
 
+def test_prepare_step_is_only_setup(md):
+    """md_prepare_step builds the graphs md_step will replay: no step is taken and the trajectory is the same bits."""
+    w = CASES["cfg3a_small"]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    x0 = a.positions()
+    a.prepare_step(37, w.dt)
+    assert np.array_equal(a.positions(), x0) and a.stats()["steps"] == 0
+    a.step(37, w.dt)
+    b.step(37, w.dt)
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    assert a.stats()["graph_active"] == 1 and a.stats()["rebuilds"] == b.stats()["rebuilds"]
+    a.set_option(md.MD_OPT_GRAPH, 0)
+    a.prepare_step(5, w.dt)                              # nothing to prepare: still fine
+    a.step(5, w.dt)
+    b.step(5, w.dt)
+    assert np.array_equal(a.positions(), b.positions())
+
+
 def test_diagnostics_run(md):
     rate, mhz = md.fp64_dfma_rate()
     assert rate > 1e12 and mhz > 500
