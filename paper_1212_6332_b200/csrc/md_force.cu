@@ -1,6 +1,8 @@
 // md_force.cu — density pass (paper's G18, Fig.5) and force pass with
-// energy and virial (paper's G22, Fig.6), FP64; one thread per atom, or 8 lanes per atom
-// for small systems (k_*_sub).
+// energy and virial (paper's G22, Fig.6), FP64; one thread per atom, or 4 / 8 / 32 lanes per
+// atom for small systems (k_*_sub); optionally as Newton's-third-law passes (HALF).
+// Inside md_step the force pass also performs both half-kicks, the next step's drift and the displacement check, and
+// its last block takes the rebuild decision (force_finish, finish_displacement).
 //
 // Differences from the paper's kernels:
 //  - atoms are in cell order and the list is a blocked-ELL array in 16-byte groups of four entries, so one LDG.128

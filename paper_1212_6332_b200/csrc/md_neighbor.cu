@@ -3,9 +3,10 @@
 // Paper: section 3.2 and Fig.3.  The paper computes only the
 // cell index on the GPU (G1-G3) and builds linked lists, sorts atoms by cell and re-sorts velocities
 // on the HOST ("due to its sequential nature").  Here the whole chain runs on the
-// device: histogram -> scan -> scatter -> per-cell ordering -> re-order -> list, and every kernel of the
-// chain is launched unconditionally but returns at once unless DevState says a rebuild is due, so that
-// md_step never needs the host to look at the displacement flag.
+// device: histogram -> scan -> scatter -> per-cell ordering -> re-order -> list.  Whether a rebuild is due is decided on
+// the device (decide_rebuild, md_internal.cuh): inside md_step's CUDA graphs the chain is the body of a conditional node;
+// launched plainly, every kernel of the chain returns at once unless DevState says a rebuild is due.  Either way md_step
+// never needs the host to look at the displacement flag.
 #include <type_traits>
 
 #include "md_internal.cuh"
