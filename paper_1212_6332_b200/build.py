@@ -12,6 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmd_b200.so")
+OBJ = os.path.join(HERE, "build")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-shared", "-cudart", "static", "--expt-relaxed-constexpr"]
@@ -27,8 +28,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     extra = os.environ.get("MD_NVCC_EXTRA", "").split()          # e.g. -DMD_FORCE_MINB=5 (tuning knobs of md_force.cu)
-    cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *sources()]
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    cflags = [f for f in FLAGS if f != "-shared"] + extra + (["-Xptxas", "-v"] if verbose else [])
+    os.makedirs(OBJ, exist_ok=True)
+    jobs = []                                                     # one nvcc per translation unit, side by side, then one link
+    for src in sources():
+        obj = os.path.join(OBJ, os.path.splitext(os.path.basename(src))[0] + ".o")
+        cmd = [NVCC, *cflags, "-c", "-o", obj, src]
+        jobs.append((cmd, obj, subprocess.Popen(cmd, cwd=CSRC)))
+    failed = [(cmd, p.returncode) for cmd, _, p in jobs if p.wait() != 0]
+    if failed:
+        raise subprocess.CalledProcessError(failed[0][1], failed[0][0])
+    subprocess.run([NVCC, *FLAGS, "-o", LIB, *(obj for _, obj, _ in jobs)], check=True, cwd=CSRC)
     return LIB
 
 
