@@ -247,6 +247,28 @@ int md_fp64_dfma_rate(void *stream, double *dfma_per_s, double *sm_clock_mhz);
  * (cudaMalloc / cudaFree inside the call) and synchronises the stream. */
 int md_probe_table_gather(void *stream, double ns_per_warp_gather[4]);
 
+/* For callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): E_kin = sum_i 1/2 m_i |v_i|^2 (the kinetic term of eq.(6); what md_get_energies reports per
+ * box) of n_atoms atoms, with NO workspace and NO allocation: the block partials of the reduction live in a file-scope
+ * device array of the library (33,024 bytes, held by every device that loads the library until the process exits), which
+ * bounds n_atoms by MD_NOALLOC_MAX_ATOMS.  Enqueues one 8-byte memset and one kernel on `stream`; calls no cudaMalloc,
+ * cudaFree or allocating library routine; does not synchronise.
+ *   stream   cudaStream_t of the CURRENT device (the scratch address is looked up per device, for the device that is
+ *            current at the call)
+ *   v        DEVICE, [n_atoms][3] A/fs (the layout of md_get_velocities)
+ *   types    DEVICE, [n_atoms] in 0..n_types-1; may be NULL when n_types == 1
+ *   mass     HOST, [n_types] amu (read during the call)
+ *   ekin     DEVICE, one double, eV: written by the kernel (n_atoms == 0 gives 0)
+ *   err      HOST, optional buffer of err_len bytes that receives a one-line message when the call fails ("" on MD_OK)
+ * Returns MD_EINVAL (NULL pointer, n_types outside 1..MD_MAX_TYPES, a mass that is not positive and finite, n_atoms < 0 or
+ * n_atoms > MD_NOALLOC_MAX_ATOMS: the message names the limit), MD_ECUDA.  The sum is deterministic (fixed order for a
+ * given n_atoms).  ALL calls on one device share the scratch array and it keeps the last call's contents (the call clears
+ * the one word that must start at zero): two calls that overlap on the GPU (different streams, or one process's threads
+ * without ordering between them) race; calls ordered on one stream do not. */
+#define MD_NOALLOC_MAX_ATOMS 4194304
+int md_kinetic_energy_noalloc(void *stream, const double *v, const int *types, const double *mass, int n_types, int n_atoms,
+                              double *ekin, char *err, int err_len);
+
 const char *md_strerror(int status);
 const char *md_version(void);
 

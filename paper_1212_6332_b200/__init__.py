@@ -88,6 +88,8 @@ def lib() -> C.CDLL:
         L.md_get_pressure.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.md_profile_read.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_long), C.POINTER(C.c_double)]
         L.md_fp64_dfma_rate.argtypes = [C.c_void_p, _D, _D]
+        L.md_kinetic_energy_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, _D, C.c_int, C.c_int, C.c_void_p,
+                                                C.c_char_p, C.c_int]
         _lib = L
     return _lib
 
@@ -131,6 +133,28 @@ def probe_table_gather():
     out = (C.c_double * 4)()
     check(lib().md_probe_table_gather(C.c_void_p(torch.cuda.current_stream().cuda_stream), out))
     return tuple(out)
+
+
+MD_NOALLOC_MAX_ATOMS = 4194304
+
+
+def kinetic_energy_noalloc(v, types, mass, out):
+    """E_kin (eV) of velocities `v` [n, 3] (torch CUDA float64) into `out` (torch CUDA float64, 1 element) without any
+    allocation on the device: the scratch is a fixed array inside the library (n <= MD_NOALLOC_MAX_ATOMS).  `types`: torch
+    CUDA int32 [n] or None for one species; `mass`: amu per type (host).  Enqueued on torch's current stream; returns `out`."""
+    import torch
+    assert v.is_cuda and v.dtype == torch.float64 and v.is_contiguous() and v.dim() == 2 and v.shape[1] == 3
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1
+    assert types is None or (types.is_cuda and types.dtype == torch.int32 and types.is_contiguous() and types.numel() == v.shape[0])
+    m = (C.c_double * len(mass))(*[float(x) for x in mass])
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(v.device):
+        rc = lib().md_kinetic_energy_noalloc(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.c_void_p(v.data_ptr()),
+                                             C.c_void_p(types.data_ptr()) if types is not None else None, m, len(mass),
+                                             int(v.shape[0]), C.c_void_p(out.data_ptr()), err, len(err))
+    if rc != MD_OK:
+        raise MDError(rc, err.value.decode() or lib().md_strerror(rc).decode())
+    return out
 
 
 class MDSystem:

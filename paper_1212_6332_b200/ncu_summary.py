@@ -44,7 +44,7 @@ TABLE = [
 def csrc_sha() -> str:
     h = hashlib.sha256()
     for f in sorted(glob.glob(os.path.join(ROOT, "paper_1212_6332_b200", "csrc", "*"))):
-        if os.path.basename(f) == "md_probe.cu":          # diagnostics only: not part of the MD path
+        if os.path.basename(f) in ("md_probe.cu", "md_noalloc.cu"):   # diagnostics / stand-alone entry points: not part of the MD path
             continue
         h.update(os.path.basename(f).encode())
         with open(f, "rb") as fh:
