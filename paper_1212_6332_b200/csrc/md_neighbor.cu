@@ -171,6 +171,10 @@ __global__ void k_copyback(const __grid_constant__ DevSys s) {
   s.orig[i] = s.orig_tmp[i];
 }
 
+#ifndef MD_LIST_MINB
+#define MD_LIST_MINB 7                           // measured on B200: 6 / 7 / 8 blocks per SM (80 / 72 / 64 registers): 0.814 / 0.784 / 0.795 ms per step on cfg4
+#endif
+
 // ---- K9: the neighbour list (paper's G6, Fig.3) ---------------------------------------------------
 // One thread per atom (as G6), but no shared-memory tiles: atoms are already in cell order, so the
 // candidates of the three z-adjacent cells of one (x,y) column are one contiguous run of slots.
@@ -190,6 +194,15 @@ __device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-
   return v;
 }
 
+// The canonical double-precision test of one candidate against r_l, with the shift of its run (d + 0.0 == d).  Out of line
+// on purpose: the float classification of k_build_list calls it for about one candidate in 10^4, and inlined it would be
+// if-converted into the candidate loop.
+__device__ __noinline__ bool exact_within(const double4 *pj_ptr, double4 pi, double sx, double sy, double sz, double rl2) {
+  const double4 pj = ld_pos(pj_ptr);
+  const double dx = __dadd_rn(__dsub_rn(pj.x, pi.x), sx), dy = __dadd_rn(__dsub_rn(pj.y, pi.y), sy), dz = __dadd_rn(__dsub_rn(pj.z, pi.z), sz);
+  return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)) < rl2;
+}
+
 // The stencil is 3 x 3 columns of cells (cell side >= r_l in x and y), each column ONE contiguous run of slots:
 // ZWIN = false: cubic cells, three cells of z per column; ZWIN = true (small boxes, DevSys::zfine > 1): thinner cells in z
 // and per atom and column the z window that r_l can reach.
@@ -198,8 +211,8 @@ __device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-
 // the branch of the canonical minimum image is decided by the pair of cells: the shift (0, -L or +L) and its image
 // code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
 // (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
-template <bool PERCELL, bool ZWIN>
-__global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constant__ DevSys s) {
+template <bool PERCELL, bool ZWIN, bool F32CLS = false>
+__global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 1) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * blockDim.x + threadIdx.x;
@@ -209,6 +222,18 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   unsigned *row = s.nbr + nbr_row_offset(tile, s.cap, local & 31);
   const double4 pi = s.pos[i];
   const double L[3] = {box_edge(s, 0), box_edge(s, 1), box_edge(s, 2)};
+  const float4 q32 = s.pos32[i];
+  // F32CLS: a candidate is classified on the float copies of the coordinates wherever that is unambiguous.  With u = 2^-24,
+  // |x| <= L and the shift rounded to float, each component of d = x_j - x_i (+ shift) is off by at most u (4 L + |d|), and
+  // r2 = fma(dz, dz, fma(dy, dy, dx dx)) by at most E(r) = 2 sqrt(3) u r (4 L + r) + 4 u r^2 < u (14 L r + 7.5 r^2);
+  // r^2 - E(r) grows with r, so a float r2 outside the band [r_l^2 - eps, r_l^2 + eps), eps = u (32 L r_l + 24 r_l^2) >=
+  // 2 E(r_l) plus the rounding of the bounds themselves, is on the same side of r_l^2 as the canonical double-precision r2
+  // of reading A3.  Inside the band (about one candidate in 10^4) the canonical test decides: the list is bit-exact either
+  // way.  The split of a row at r_in only orders it (both parts of a row are tested against r_c by the passes): it is taken
+  // from the float.
+  const double eps32 = 5.9604644775390625e-8 * (32.0 * fmax(fmax(L[0], L[1]), L[2]) * s.rl + 24.0 * s.rl2);
+  const float rl2_lo = (float)(s.rl2 - eps32), rl2_hi = (float)(s.rl2 + eps32), rl2_below = __int_as_float(__float_as_int(rl2_lo) - 1);
+  const float rin2f = fminf((float)s.rin2, rl2_below);
   const int cx = cell_coord(pi.x, s.nc[0] / L[0], s.nc[0]);
   const int cy = cell_coord(pi.y, s.nc[1] / L[1], s.nc[1]);
   const int cz = cell_coord(pi.z, s.nc[2] / L[2], s.nc[2]);
@@ -223,9 +248,9 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   // append would run for the whole warp on nearly every candidate
   int n_lost = 0;                                                 // accepted but not stored (row full)
   int m_out = s.cap - 1;                                          // next free entry from the back (n_out = cap - 1 - m_out)
-  auto test_keep = [&](int j, double r2, unsigned code) {
-    const bool acc = r2 < s.rl2 && j != i;
-    const bool in = r2 < s.rin2;
+  // keep(j, inside r_l, inside r_in, image code): the append; test_keep: the canonical double-precision decision first
+  auto keep = [&](int j, bool within, bool in, unsigned code) {
+    const bool acc = within && j != i;
     const bool put = acc && n_in <= m_out;                        // room: n_in + n_out < cap
     const int k = in ? n_in : m_out;
     // one predicated store, no branch: address = row + 4 * offset by one 32 x 32 -> 64 bit multiply-add
@@ -235,6 +260,7 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
     m_out -= (put && !in) ? 1 : 0;
     n_lost += (acc && !put) ? 1 : 0;
   };
+  auto test_keep = [&](int j, double r2, unsigned code) { keep(j, r2 < s.rl2, r2 < s.rin2, code); };
   // candidates of the slot range [jbeg, jend), all with the same periodic shift (sx, sy, sz) / image code
   auto scan_range = [&](int jbeg, int jend, double sx, double sy, double sz, unsigned code) {
     if (PERCELL) {
@@ -260,7 +286,41 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
           test_keep(j, r2, code);
         }
       };
-      if (code) scan(std::true_type{}); else scan(std::false_type{});
+      // the same runs on the float copies (16 bytes per candidate instead of 32, no FP64 instruction outside the band)
+      auto scan32 = [&](auto shifted) {
+        const float fx = (float)sx, fy = (float)sy, fz = (float)sz;
+        auto ld32 = [&](int j) {
+          float4 v;
+          asm("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(s.pos32 + j));
+          return v;
+        };
+        auto dist2f = [&](const float4 &a) {
+          float dx = a.x - q32.x, dy = a.y - q32.y, dz = a.z - q32.z;
+          if (decltype(shifted)::value) { dx += fx; dy += fy; dz += fz; }
+          return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        };
+        auto in_band = [&](float r2) { return !(r2 < rl2_lo) && r2 < rl2_hi; };
+        // a candidate in the band gets the canonical test (reading A3) and leaves with an r2 outside the band, on the side
+        // that test found: the decision below is then taken from the float alone, for every candidate alike
+        auto settle = [&](int j, float &r2) {
+          if (in_band(r2)) r2 = exact_within(s.pos + j, pi, sx, sy, sz, s.rl2) ? rl2_below : rl2_hi;
+        };
+        int j = jbeg;
+        for (; j + 4 <= jend; j += 4) {
+          const float4 a0 = ld32(j), a1 = ld32(j + 1), a2 = ld32(j + 2), a3 = ld32(j + 3);
+          float r0 = dist2f(a0), r1 = dist2f(a1), r2 = dist2f(a2), r3 = dist2f(a3);
+          if (in_band(r0) | in_band(r1) | in_band(r2) | in_band(r3)) { settle(j, r0); settle(j + 1, r1); settle(j + 2, r2); settle(j + 3, r3); }
+          keep(j, r0 < rl2_lo, r0 < rin2f, code); keep(j + 1, r1 < rl2_lo, r1 < rin2f, code);
+          keep(j + 2, r2 < rl2_lo, r2 < rin2f, code); keep(j + 3, r3 < rl2_lo, r3 < rin2f, code);
+        }
+        for (; j < jend; ++j) {
+          float r2 = dist2f(ld32(j));
+          settle(j, r2);
+          keep(j, r2 < rl2_lo, r2 < rin2f, code);
+        }
+      };
+      if constexpr (F32CLS) { if (code) scan32(std::true_type{}); else scan32(std::false_type{}); }
+      else { if (code) scan(std::true_type{}); else scan(std::false_type{}); }
     } else {
       // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
       auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
@@ -346,7 +406,6 @@ __global__ void __launch_bounds__(kForceBlock) k_build_list(const __grid_constan
   // copies of the coordinates (pos32, written with the re-order) against r_l^2 plus a margin that covers the rounding of
   // the copies (|x| <= L: 2^-24 L per coordinate), so no pair of the list can be missed.  The survivors (the list plus
   // about one candidate in 10^4) are parked in the row itself, in scan order.
-  const float4 q32 = s.pos32[i];
   const float Lf[3] = {(float)L[0], (float)L[1], (float)L[2]}, iLf[3] = {1.f / Lf[0], 1.f / Lf[1], 1.f / Lf[2]};
   const float rl2f = (float)s.rl2 + 4e-6f * (float)s.rl * (fmaxf(fmaxf(Lf[0], Lf[1]), Lf[2]) + (float)s.rl);
   int ns = 0, ns_own = 0;
@@ -524,7 +583,11 @@ int launch_rebuild_body(md_system *sys) {
     if (d.zfine > 1) {
       if (percell) k_build_list<true, true><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, true><<<gl, kForceBlock, 0, st>>>(d);
     } else {
-      if (percell) k_build_list<true, false><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, false><<<gl, kForceBlock, 0, st>>>(d);
+      // large boxes: classification on the float copies (MD_LIST_F64: the double-precision scan, for the measurement in DESIGN.md)
+      static const bool f64 = getenv("MD_LIST_F64") != nullptr;
+      if (percell && !f64) k_build_list<true, false, true><<<gl, kForceBlock, 0, st>>>(d);
+      else if (percell) k_build_list<true, false><<<gl, kForceBlock, 0, st>>>(d);
+      else k_build_list<false, false><<<gl, kForceBlock, 0, st>>>(d);
     }
   }
   return (int)cudaGetLastError();
