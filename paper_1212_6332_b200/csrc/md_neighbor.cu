@@ -212,7 +212,7 @@ __device__ __noinline__ bool exact_within(const double4 *pj_ptr, double4 pi, dou
 // code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
 // (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
 template <bool PERCELL, bool ZWIN, bool F32CLS = false>
-__global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 1) k_build_list(const __grid_constant__ DevSys s) {
+__global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 0) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
   const int box = blockIdx.x / bpb, local = (blockIdx.x - box * bpb) * blockDim.x + threadIdx.x;
