@@ -643,6 +643,36 @@ def test_error_codes(md):
     assert ei.value.code == md.MD_ESTATE
 
 
+def test_list_build_at_the_edge_of_the_list_cutoff(md):
+    """Pairs whose separation straddles r_l = r_c + skin by relative amounts from 1e-16 to 1e-5, at coordinates up to 590 A
+    (where a float coordinate is rounded by up to 3e-5 A) and across the periodic boundary.  In boxes of this size the list
+    build classifies the candidates on float copies of the coordinates and takes the canonical double-precision test
+    (reading A3) inside the rounding band only (md_neighbor.cu): the pair sets must still be the
+    oracle's, which takes every decision in double precision (brute force over all pairs here)."""
+    rng = np.random.default_rng(12126332 + 77)
+    L, rc, skin, K = 590.0, 4.9, 0.3, 3000
+    rl = rc + skin
+    a = rng.uniform(0.0, L, (K, 3))
+    face = rng.integers(0, 3, K // 4)                                         # a quarter of the pairs at a face of the box
+    a[np.arange(K // 4), face] = np.where(rng.random(K // 4) < 0.5, rng.uniform(0.0, 2.0, K // 4), rng.uniform(L - 2.0, L, K // 4))
+    u = rng.normal(size=(K, 3))
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    delta = 10.0 ** rng.uniform(-16.0, -5.0, K) * rng.choice([-1.0, 1.0], K)
+    delta[:50] = 0.0                                                          # as close to r_l as the rounding of b allows
+    b = a + (rl * (1.0 + delta))[:, None] * u                                 # some b lie outside [0, L): the build wraps them
+    pos = np.concatenate([a, b])
+    kw = dict(box=np.full(3, L), cutoff=rc, skin=skin, n_boxes=1, pot_kind=0, mass=np.array([63.546]), tbsma=workloads.cu_tbsma_params(rc),
+              positions=pos, types=np.zeros(2 * K, np.int32))
+    o = oracle_of(None, velocities=np.zeros_like(pos), **kw)
+    o.build_neighbors(brute_force=True)
+    oc, ol = o.neighbors(stride=16)
+    g = md.MDSystem(velocities=None, **kw)
+    g.build_neighbors()
+    gc, gl = g.neighbors(stride=16)
+    assert np.array_equal(gc, oc) and np.array_equal(gl, ol)
+    assert 0.3 * K < oc[:K].sum() < 0.7 * K and g.stats()["error_flags"] == 0   # about half of the pairs are listed: the edge is straddled
+
+
 def test_sparse_and_tiny_systems(md):
     """degenerate inputs: atoms with no neighbour at all, a box holding two atoms, a one-atom box batch."""
     base = dict(box=np.full(3, 40.0), velocities=None, cutoff=4.9, skin=0.3, n_boxes=1, pot_kind=0,
