@@ -220,8 +220,8 @@ int md_get_stats(md_system *s, md_stats *st);         /* synchronises */
  *                           gathers, not by arithmetic), 0 for MD_POT_TBSMA (full lists, as the paper's GPU kernels). */
 enum { MD_OPT_STEP_OBSERVABLES = 1, MD_OPT_PROFILE = 2, MD_OPT_FORCE_VARIANT = 3, MD_OPT_GRAPH = 4, MD_OPT_HALF_LIST = 5 };
 /* Three environment variables select variants that DESIGN.md section 6 measures against the defaults (read by md_create /
- * at the first md_step / at the first list build; results do not depend on them): MD_LIST_F64 (the list build of large boxes
- * tests every candidate in double precision instead of classifying it on float copies of the coordinates first), MD_CELL_ZFINE = 1, 2, 4 (cells thinner in z by that factor and a z
+ * at the first md_step / at the first list build; results do not depend on them): MD_LIST_F64 (the list build tests every
+ * candidate in double precision instead of classifying it on float copies of the coordinates first), MD_CELL_ZFINE = 1, 2, 4 (cells thinner in z by that factor and a z
  * window per column in the list build; default 4 in boxes with an edge shorter than 5 (cutoff + skin), else 1) and
  * MD_NO_LOOP_GRAPH (per-step IF nodes also for small systems).  MD_DEBUG prints why a CUDA graph could not be built. */
 int md_set_option(md_system *s, int option, int value);

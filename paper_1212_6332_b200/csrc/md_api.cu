@@ -77,10 +77,10 @@ static int geometry(const md_desc *d, Geometry &g, bool check_pairs) {
     if (g.nc[a] < 3) return MD_EBOX;                 // 26 distinct neighbour cells
     vol *= d->box[a];
   }
-  // Small boxes (some edge shorter than 5 r_l: the image of a pair is decided per pair, and the build filters in single
-  // precision): cells four times thinner in z (the fastest cell index: a column of cells is one contiguous run of slots).
-  // The candidates of a column are then the z window [z_i - w, z_i + w], w^2 = r_l^2 - (lateral gap to the column)^2,
-  // instead of three whole cells: cfg2 list build 0.094 -> 0.082 ms per step.  Large boxes keep cubic cells: there the
+  // Small boxes (some edge shorter than 5 r_l): cells four times thinner in z (the fastest cell index: a column of cells is
+  // one contiguous run of slots).  The candidates of a column are then the z window [z_i - w, z_i + w], w^2 = r_l^2 -
+  // (lateral gap to the column)^2, instead of three whole cells: cfg2 list build 0.097 (cubic cells) / 0.088 (half) / 0.081
+  // (quarter cells) ms per step with the list kernel of md_neighbor.cu.  Large boxes keep cubic cells: there the
   // lanes of a warp that share a cell scan the SAME slots (their loads are broadcasts), and per-atom windows cost more in
   // L1 wavefronts than they save in tests (measured: 0.58 -> 0.70 ms per 1 M atoms with quarter cells, 0.61 with half).
   // Also measured and dropped: cells of half the cut-off in all three directions with a 5 x 5 x 5 stencil (0.76 ms).

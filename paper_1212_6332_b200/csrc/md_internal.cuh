@@ -82,7 +82,7 @@ struct DevSys {
   // per-atom state, CELL ORDER (index = "slot")
   double4 *pos;                    // x,y,z, w = type as double
   double4 *posf;                   // x,y,z, w = F'(rho): written by the density pass, gathered by the force pass
-  float4 *pos32;                   // x,y,z rounded to float at the last re-order: the list build's single-precision filter
+  float4 *pos32;                   // x,y,z rounded to float at the last re-order: the list build classifies its candidates on these
   double *vel, *frc, *xref;        // SoA, component c at [c*N + i]
   double *gacc, *gjrk, *gsnp;      // Gear predictor-corrector (md_gear.cu): second, third and fourth time derivative of x, SoA
   int *type, *orig;                // orig = caller index of the atom in this slot (paper's hGID)

@@ -181,13 +181,6 @@ __global__ void k_copyback(const __grid_constant__ DevSys s) {
 // The pair test is the canonical minimum image + non-contracted r2, so the sets are bit-exact.
 // Each entry records which image was taken (2 bits per axis) so that the density and force passes
 // can form the SAME d = (x_j - x_i) -/+ L without re-deciding.
-__device__ __forceinline__ double min_image(double d, double L, double hL, unsigned &code) {
-  code = 0;
-  if (d > hL) { d = __dsub_rn(d, L); code = 2; }          // took  d - L
-  else if (d < -hL) { d = __dadd_rn(d, L); code = 1; }    // took  d + L
-  return d;
-}
-
 __device__ __forceinline__ double4 ld_pos(const double4 *p) {        // one 256-bit load on the read-only path
   double4 v;
   asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
@@ -206,12 +199,17 @@ __device__ __noinline__ bool exact_within(const double4 *pj_ptr, double4 pi, dou
 // The stencil is 3 x 3 columns of cells (cell side >= r_l in x and y), each column ONE contiguous run of slots:
 // ZWIN = false: cubic cells, three cells of z per column; ZWIN = true (small boxes, DevSys::zfine > 1): thinner cells in z
 // and per atom and column the z window that r_l can reach.
-// PERCELL (every edge >= 5 r_l): two atoms of neighbouring cells WITHOUT crossing the box boundary are closer than
-// 0.4 L per axis, and two atoms of cells that are neighbours ACROSS the boundary differ by more than 0.6 L, so
-// the branch of the canonical minimum image is decided by the pair of cells: the shift (0, -L or +L) and its image
-// code are set once per run of candidates, and d = (x_j - x_i) + shift is bit-identical to the canonical value
-// (d + 0.0 == d, d + (-L) == d - L).  This takes the two compares and the selects per axis out of the candidate loop.
-template <bool PERCELL, bool ZWIN, bool F32CLS = false>
+// The periodic image is decided per RUN of candidates, not per pair: a run that lies across the box boundary carries the
+// shift (-L or +L per axis) and its image code, and d = (x_j - x_i) + shift.  For every pair that can be accepted this is
+// the canonical minimum image of reading A3, bit for bit (d + 0.0 == d, d + (-L) == d - L): an accepted pair has
+// |d_a + shift_a| < r_l <= L/3 on every axis, so that image IS the one the canonical rule picks; and a candidate whose
+// canonical image differs from its run's has |d_a + shift_a| > L/2 there and, since the two cells are neighbours (at most
+// two cell widths apart), its canonical component is longer than L - 2 L/nc >= one cell width >= r_l: rejected either way
+// (every edge holds at least three cells, MD_EBOX otherwise).  This takes the compares and selects of the minimum image
+// out of the candidate loop.  (Up to round 2 boxes with fewer than five cells per edge took the minimum image per pair,
+// behind a single-precision filter and a second phase over the survivors; the per-run form with the float
+// classification below replaced it: cfg2 list build 0.0827 -> 0.0806 ms per step, cfg0 0.0084 -> 0.0079.)
+template <bool ZWIN, bool F32CLS>
 __global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 0) k_build_list(const __grid_constant__ DevSys s) {
   if (!s.st->do_rebuild) return;
   const int bpb = (s.npb + blockDim.x - 1) / blockDim.x;
@@ -263,7 +261,7 @@ __global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 0) k_buil
   auto test_keep = [&](int j, double r2, unsigned code) { keep(j, r2 < s.rl2, r2 < s.rin2, code); };
   // candidates of the slot range [jbeg, jend), all with the same periodic shift (sx, sy, sz) / image code
   auto scan_range = [&](int jbeg, int jend, double sx, double sy, double sz, unsigned code) {
-    if (PERCELL) {
+    {
       // four candidates per trip: the four loads are issued together (read-only path, so the list stores
       // in between cannot hold them back), then the four tests
       // runs across the box boundary add the shift (d + (-L) == d - L bit for bit); the others (95 % in a large box) do not
@@ -321,30 +319,6 @@ __global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 0) k_buil
       };
       if constexpr (F32CLS) { if (code) scan32(std::true_type{}); else scan32(std::false_type{}); }
       else { if (code) scan(std::true_type{}); else scan(std::false_type{}); }
-    } else {
-      // small boxes (some nc < 5): the canonical minimum image per pair (reading A3), four candidates per trip
-      auto dist2m = [&](const double4 &pj, double &r2, unsigned &code) {
-        unsigned ax, ay, az;
-        const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
-        const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
-        const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
-        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-        code = ax | (ay << 2) | (az << 4);
-      };
-      int j = jbeg;
-      for (; j + 4 <= jend; j += 4) {
-        const double4 p0 = ld_pos(s.pos + j), p1 = ld_pos(s.pos + j + 1), p2 = ld_pos(s.pos + j + 2), p3 = ld_pos(s.pos + j + 3);
-        double r0, r1, r2, r3;
-        unsigned c0, c1, c2, c3;
-        dist2m(p0, r0, c0); dist2m(p1, r1, c1); dist2m(p2, r2, c2); dist2m(p3, r3, c3);
-        test_keep(j, r0, c0); test_keep(j + 1, r1, c1); test_keep(j + 2, r2, c2); test_keep(j + 3, r3, c3);
-      }
-      for (; j < jend; ++j) {
-        double r2;
-        unsigned c;
-        dist2m(ld_pos(s.pos + j), r2, c);
-        test_keep(j, r2, c);
-      }
     }
   };
   // One (x, y) column of the stencil: up to three runs of slots: the in-range z cells (contiguous), plus the wrapped cell
@@ -402,90 +376,7 @@ __global__ void __launch_bounds__(kForceBlock, F32CLS ? MD_LIST_MINB : 0) k_buil
   };
   int n_own_in = 0, n_own_out = 0;
 
-  // ---- Phase 1: single-precision filter.  9 of 10 candidates of the 27 cells are beyond r_l; they are rejected on float
-  // copies of the coordinates (pos32, written with the re-order) against r_l^2 plus a margin that covers the rounding of
-  // the copies (|x| <= L: 2^-24 L per coordinate), so no pair of the list can be missed.  The survivors (the list plus
-  // about one candidate in 10^4) are parked in the row itself, in scan order.
-  const float Lf[3] = {(float)L[0], (float)L[1], (float)L[2]}, iLf[3] = {1.f / Lf[0], 1.f / Lf[1], 1.f / Lf[2]};
-  const float rl2f = (float)s.rl2 + 4e-6f * (float)s.rl * (fmaxf(fmaxf(Lf[0], Lf[1]), Lf[2]) + (float)s.rl);
-  int ns = 0, ns_own = 0;
-  bool exact_path = false;                                        // the row cannot hold the survivors: classify during the scan instead
-  auto park = [&](int j, float r2, unsigned code) {
-    const bool hit = r2 < rl2f && j != i;
-    const bool put = hit && ns < s.cap;
-    asm volatile("{\n\t.reg .pred p;\n\t.reg .u64 a;\n\tsetp.ne.u32 p, %3, 0;\n\tmad.wide.u32 a, %1, 4, %0;\n\t@p st.global.u32 [a], %2;\n\t}"
-                 :: "l"((unsigned long long)row), "r"(nbr_entry(ns)), "r"((unsigned)j | (code << kIdxBits)), "r"((unsigned)put) : "memory");
-    ns += put ? 1 : 0;
-    exact_path |= hit && !put;
-  };
-  auto filter_range = [&](int jbeg, int jend, double sx, double sy, double sz, unsigned code) {
-    auto ld32 = [&](int j) {
-      float4 v;
-      asm("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(s.pos32 + j));
-      return v;
-    };
-    const float fx = (float)sx, fy = (float)sy, fz = (float)sz;
-    auto dist2f = [&](const float4 &a) {
-      float dx = a.x - q32.x, dy = a.y - q32.y, dz = a.z - q32.z;
-      if (PERCELL) { dx += fx; dy += fy; dz += fz; }
-      else {                                                      // nearest image: either image is beyond r_l when they tie (L >= 3 r_l)
-        dx -= Lf[0] * rintf(dx * iLf[0]); dy -= Lf[1] * rintf(dy * iLf[1]); dz -= Lf[2] * rintf(dz * iLf[2]);
-      }
-      return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    };
-    int j = jbeg;
-    for (; j + 4 <= jend; j += 4) {
-      const float4 a0 = ld32(j), a1 = ld32(j + 1), a2 = ld32(j + 2), a3 = ld32(j + 3);
-      const float r0 = dist2f(a0), r1 = dist2f(a1), r2 = dist2f(a2), r3 = dist2f(a3);
-      park(j, r0, code); park(j + 1, r1, code); park(j + 2, r2, code); park(j + 3, r3, code);
-    }
-    for (; j < jend; ++j) park(j, dist2f(ld32(j)), code);
-  };
-  // Measured on B200: a gain only where the exact test is expensive (small boxes: minimum image per pair, cfg2 list build
-  // 0.140 -> 0.094 ms per step); in large boxes (PERCELL) the scan's loads are broadcasts within a cell while the second
-  // phase gathers one position per survivor and lane, and the L1 data pipe makes the build 20 % SLOWER (0.58 -> 0.70 ms per
-  // 1 M atoms): there every candidate is classified in double precision during the scan, as in round 1.
-  if constexpr (PERCELL) exact_path = true;
-  else stencil(filter_range, [&]() { ns_own = ns; });
-
-  // ---- Phase 2: the survivors, in the same order, with the canonical double-precision test (reading A3); accepted
-  // entries go back into the row from both ends (the front never overtakes the reader)
-  if (!exact_path) {
-    for (int t = 0; t < ns; ++t) {
-      if (t == ns_own) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
-      const unsigned e = row[nbr_entry(t)];
-      const int j = (int)(e & kIdxMask);
-      const double4 pj = ld_pos(s.pos + j);
-      double r2;
-      unsigned code;
-      if (PERCELL) {
-        code = e >> kIdxBits;
-        double dx = __dsub_rn(pj.x, pi.x), dy = __dsub_rn(pj.y, pi.y), dz = __dsub_rn(pj.z, pi.z);
-        if (code) {                                               // the shifts of the run this candidate came from (0.0 where none)
-          dx = __dadd_rn(dx, (code & 1u) ? L[0] : ((code & 2u) ? -L[0] : 0.0));
-          dy = __dadd_rn(dy, (code & 4u) ? L[1] : ((code & 8u) ? -L[1] : 0.0));
-          dz = __dadd_rn(dz, (code & 16u) ? L[2] : ((code & 32u) ? -L[2] : 0.0));
-        }
-        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      } else {
-        unsigned ax, ay, az;
-        const double dx = min_image(__dsub_rn(pj.x, pi.x), L[0], 0.5 * L[0], ax);
-        const double dy = min_image(__dsub_rn(pj.y, pi.y), L[1], 0.5 * L[1], ay);
-        const double dz = min_image(__dsub_rn(pj.z, pi.z), L[2], 0.5 * L[2], az);
-        r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-        code = ax | (ay << 2) | (az << 4);
-      }
-      if (r2 < s.rl2 && !(r2 < s.rin2) && m_out > t && m_out < ns) { exact_path = true; break; }   // the back would overwrite unread survivors
-      test_keep(j, r2, code);
-    }
-    if (ns_own >= ns) { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; }
-  }
-  // ---- Rows too full for that (a capacity close to the row length, or an overflow): every candidate classified in double
-  // precision during the scan, which also counts what does not fit
-  if (exact_path) {
-    n_in = 0; m_out = s.cap - 1; n_lost = 0;
-    stencil(scan_range, [&]() { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; });
-  }
+  stencil(scan_range, [&]() { n_own_in = n_in; n_own_out = s.cap - 1 - m_out; });
   n_out = s.cap - 1 - m_out;
   n_all += n_in + n_out + n_lost;
   if (n_lost > 0) atomicOr(&s.st->error_flags, MD_FLAG_OVERFLOW);
@@ -577,17 +468,13 @@ int launch_rebuild_body(md_system *sys) {
   {
     ProfScope p(sys, MD_K_LIST);
     const int gl = d.nb * blocks_per_box(d.npb, kForceBlock);
-    // edges (in units of r_l) from which the image of a pair is decided by its pair of cells
-    const bool percell = d.nc[0] >= 5 && d.nc[1] >= 5 && d.nc[2] >= 5 * d.zfine;
+    // MD_LIST_F64: every candidate tested in double precision (for the measurement in DESIGN.md section 6)
+    const bool f64 = getenv("MD_LIST_F64") != nullptr;
     ++sys->launches;
     if (d.zfine > 1) {
-      if (percell) k_build_list<true, true><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, true><<<gl, kForceBlock, 0, st>>>(d);
+      if (f64) k_build_list<true, false><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<true, true><<<gl, kForceBlock, 0, st>>>(d);
     } else {
-      // large boxes: classification on the float copies (MD_LIST_F64: the double-precision scan, for the measurement in DESIGN.md)
-      static const bool f64 = getenv("MD_LIST_F64") != nullptr;
-      if (percell && !f64) k_build_list<true, false, true><<<gl, kForceBlock, 0, st>>>(d);
-      else if (percell) k_build_list<true, false><<<gl, kForceBlock, 0, st>>>(d);
-      else k_build_list<false, false><<<gl, kForceBlock, 0, st>>>(d);
+      if (f64) k_build_list<false, false><<<gl, kForceBlock, 0, st>>>(d); else k_build_list<false, true><<<gl, kForceBlock, 0, st>>>(d);
     }
   }
   return (int)cudaGetLastError();
