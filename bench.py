@@ -353,13 +353,12 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
         Ke = min(K, args.e2e_steps) if args.e2e_steps else K
         g.prepare_step(1, w.dt)
         for _ in range(3):
-            g.set_state(hxn, hvn); g.step(1, w.dt); g.get_state(out=(hxn, hvn))
+            g.set_state(hxn, hvn); g.step_get_state(1, w.dt, out=(hxn, hvn))
         barrier()
         t0 = time.perf_counter()
         for _ in range(Ke):
             g.set_state(hxn, hvn)
-            g.step(1, w.dt)
-            g.get_state(out=(hxn, hvn))
+            g.step_get_state(1, w.dt, out=(hxn, hvn))
         barrier()
         te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
         if world > 1:
@@ -367,7 +366,8 @@ def cuda_arm(args, rank: int, world: int, local_rank: int):
         e2e = {"value": world * n * Ke / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
                "steps": Ke, "ms_per_step": 1e3 * float(te.item()) / Ke,
                "what": "per step: md_set_state(x, v) from pinned host arrays (48 B per atom host->device; the forces stay valid when "
-                       "the uploaded coordinates are the resident ones), md_step(1), md_get_state(x, v) (48 B per atom device->host)"}
+                       "the uploaded coordinates are the resident ones), md_step_get_state(1, dt, x, v) (one step; 48 B per atom device->host, the "
+                       "positions copied beside the two passes of the step, the velocities after them)"}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -182,6 +182,14 @@ int md_set_velocities(md_system *s, const double *v);
  * when x is given (it reads that flag). */
 int md_set_state(md_system *s, const double *x, const double *v);
 int md_get_state(md_system *s, double *x, double *v);
+/* md_step(n, dt) and md_get_state(x, v) in one call (sec. 3.3; n >= 1, x or v may be NULL): the same
+ * kernels in the same order and the same results, bit for bit.  When x is a host buffer (pinned, for the copy to be
+ * asynchronous) the positions of the last step are gathered and copied on a second stream right after its drift and
+ * rebuild, beside its density and force pass, which only the velocities wait for; below 262,144 atoms (where the copy is
+ * shorter than the launch overhead it hides behind; environment variable MD_FORK_MIN_ATOMS), with a barostat, the
+ * predictor-corrector integrator or MD_OPT_PROFILE it is md_step followed by md_get_state.  Creates one stream and two
+ * events at its first forked call (no device memory); synchronises. */
+int md_step_get_state(md_system *s, int n, double dt, double *x, double *v);
 /* Test hook: the list as ORIGINAL (caller) indices, ascending per atom.  count [n_atoms], list [n_atoms][stride]
  * (each row padded with -1); MD_ESTATE before the first build, MD_EOVERFLOW if some count exceeds stride. */
 int md_get_neighbors(md_system *s, int *count, int *list, int stride);

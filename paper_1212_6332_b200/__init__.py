@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
         for name in ("md_set_state", "md_get_state"):
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.md_step_get_state.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
         L.md_get_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.md_get_densities.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.md_get_energies.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -273,6 +274,12 @@ class MDSystem:
         x, v = out if out is not None else (self._out((self.n_atoms, 3), np.float64, device_out),
                                             self._out((self.n_atoms, 3), np.float64, device_out))
         check(lib().md_get_state(self._h, _ptr(x), _ptr(v)))
+        return x, v
+
+    def step_get_state(self, n: int, dt: float, device_out: bool = False, out=None):
+        x, v = out if out is not None else (self._out((self.n_atoms, 3), np.float64, device_out),
+                                            self._out((self.n_atoms, 3), np.float64, device_out))
+        check(lib().md_step_get_state(self._h, int(n), float(dt), _ptr(x), _ptr(v)))
         return x, v
 
     def neighbors(self, stride: int = 256, device_out: bool = False):

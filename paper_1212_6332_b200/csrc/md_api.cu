@@ -574,6 +574,7 @@ int md_create(const md_desc *d, void *workspace, size_t bytes, md_system **out) 
   for (auto &g : s->sg) { g.graph = nullptr; g.exec = nullptr; g.dt = 0.0; g.obs = false; g.loop = false; g.nsteps = 0; g.kernels = 0; g.iter_kernels = 0; }
   s->body_kernels = 0;
   s->graph_error = 0; s->last_step_graph = false; s->frc_keep = false;
+  s->side = nullptr; s->ev_fork = nullptr; s->ev_join = nullptr; s->side_ready = false;
   layout(d, g, workspace, s);
   DevSys &o = s->d;
   o.N = d->n_atoms; o.nb = d->n_boxes; o.npb = g.npb; o.nt = d->n_types; o.kind = d->pot_kind;
@@ -675,6 +676,7 @@ int md_destroy(md_system *s) {
   if (!s) return MD_OK;
   cudaStreamSynchronize(s->stream);
   for (auto &p : s->prof) for (cudaEvent_t ev : p.ev) cudaEventDestroy(ev);
+  if (s->side_ready) { cudaStreamSynchronize(s->side); cudaEventDestroy(s->ev_fork); cudaEventDestroy(s->ev_join); cudaStreamDestroy(s->side); }
   drop_step_graph(s);
   delete s;
   return MD_OK;
@@ -930,6 +932,53 @@ int md_get_state(md_system *s, double *x, double *v) {
   }
   if (cudaGetLastError() != cudaSuccess) return MD_ECUDA;
   return host ? sync_and_flags(s) : MD_OK;
+}
+
+// n steps and the state after them in one call.  The positions of step n are final after its drift (and the rebuild, which
+// re-orders them), while its two passes only produce the forces for the second half-kick: their gather into caller order
+// and their copy to the host run on a second stream BESIDE the density and the force pass of the last step (25 MB and
+// ~0.47 ms each for 1,048,576 atoms: the download of x disappears behind the passes).  Same kernels, same order, same bits as
+// md_step(n) followed by md_get_state; the last step is launched plainly (the fork sits between two kernels of a step).
+int md_step_get_state(md_system *s, int n, double dt, double *x, double *v) {
+  if (!s || n < 1 || !isfinite(dt) || (!x && !v)) return MD_EINVAL;
+  int rc;
+  // below ~0.26 M atoms the copy is shorter than what the plainly launched step costs more than its CUDA graph (864 atoms: 0.124
+  // against 0.101 ms per step end to end); MD_FORK_MIN_ATOMS overrides the threshold (tests)
+  const char *env = getenv("MD_FORK_MIN_ATOMS");
+  const long fork_min = env ? atol(env) : 262144;
+  const bool fork = x && !on_device(x) && s->integrator == MD_INT_VERLET && !(s->baro_tau > 0.0) && !s->opt_profile && s->d.N >= fork_min;
+  if (!fork) return (rc = md_step(s, n, dt)) != MD_OK ? rc : md_get_state(s, x, v);
+  if (n > 1 && (rc = md_step(s, n - 1, dt)) != MD_OK) return rc;
+  if (!s->have_list && (rc = request_rebuild(s)) != MD_OK) return rc;
+  if (!s->forces_valid && (rc = forces_sequence(s, s->opt_step_obs, 0.0)) != MD_OK) return rc;
+  if (!s->side_ready) {
+    int lo = 0, hi = 0;
+    if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess || cudaStreamCreateWithPriority(&s->side, cudaStreamNonBlocking, hi) != cudaSuccess)
+      return MD_ECUDA;
+    if (cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) != cudaSuccess || cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) != cudaSuccess)
+      return MD_ECUDA;
+    s->side_ready = true;
+  }
+  const DevSys &o = s->d;
+  const size_t bytes = 3 * (size_t)o.N * sizeof(double);
+  const bool obs = s->opt_step_obs;
+  cudaGraphConditionalHandle none{};
+  const StepCtl ctl = make_ctl(s, dt, none, false, false);
+  if (launch_kick_drift(s, dt, ctl) != 0 || launch_rebuild_body(s) != 0) return MD_ECUDA;
+  if (cudaEventRecord(s->ev_fork, s->stream) != cudaSuccess || cudaStreamWaitEvent(s->side, s->ev_fork, 0) != cudaSuccess) return MD_ECUDA;
+  ++s->launches, k_get_pos<<<grid_for(o.N), 256, 0, s->side>>>(o, (double *)s->stage);
+  if (cudaMemcpyAsync(x, s->stage, bytes, cudaMemcpyDeviceToHost, s->side) != cudaSuccess || cudaEventRecord(s->ev_join, s->side) != cudaSuccess) return MD_ECUDA;
+  if (launch_density(s) != 0 || launch_force(s, obs, 0.5 * dt, &ctl) != 0) return MD_ECUDA;
+  s->have_list = true; s->forces_valid = true; s->observables_valid = obs; s->last_step_graph = false; s->frc_keep = false;
+  s->steps += 1;
+  if (v) {
+    const bool dev = on_device(v);
+    double *dst = dev ? v : (double *)((char *)s->stage + bytes);
+    ++s->launches, k_get_vec<<<grid_for(o.N), 256, 0, s->stream>>>(o, o.vel, dst);
+    if (!dev && cudaMemcpyAsync(v, dst, bytes, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return MD_ECUDA;
+  }
+  if (cudaStreamWaitEvent(s->stream, s->ev_join, 0) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MD_ECUDA;
+  return sync_and_flags(s);
 }
 
 int md_set_velocities(md_system *s, const double *v) {

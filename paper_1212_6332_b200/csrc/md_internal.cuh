@@ -210,6 +210,9 @@ struct md_system {
   long steps, launches;
   double exp_tab_host[md::kExpTabLen];
   void *stage; size_t stage_bytes; // staging area for host<->device copies (inside the workspace)
+  // md_step_get_state: a second stream (highest priority) and two events, created at its first call, so that the download of the
+  // positions runs beside the two passes of the last step
+  cudaStream_t side; cudaEvent_t ev_fork, ev_join; bool side_ready;
   md::ProfClass prof[MD_K_COUNT];
 };
 

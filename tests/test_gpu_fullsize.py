@@ -148,3 +148,24 @@ def test_maximum_atom_count(md):
     del f, e
     g.step(2, w.dt)
     assert g.stats()["error_flags"] == 0 and g.stats()["steps"] == 2
+
+
+def test_end_to_end_calls_at_the_bench_size(md):
+    """bench.py's end-to-end leg at its own size (1,048,576 atoms: md_step_get_state forks the download of the positions off
+    beside the two passes): md_set_state + md_step_get_state per step give the trajectory of md_step, bit for bit."""
+    import torch
+    w = workloads.config("3a")
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    n = w.n_atoms
+    hx, hv = torch.empty((n, 3), dtype=torch.float64).pin_memory().numpy(), torch.empty((n, 3), dtype=torch.float64).pin_memory().numpy()
+    b.get_state(out=(hx, hv))
+    a.step(16, w.dt)
+    for _ in range(16):
+        b.set_state(hx, hv)
+        b.step_get_state(1, w.dt, out=(hx, hv))
+    xa, va = a.get_state()
+    assert np.array_equal(xa, hx) and np.array_equal(va, hv)
+    assert a.stats()["rebuilds"] == b.stats()["rebuilds"] >= 2 and b.stats()["error_flags"] == 0
+    a.step(5, w.dt)
+    xb, vb = b.step_get_state(5, w.dt, out=(hx, hv))
+    assert np.array_equal(a.positions(), xb) and np.array_equal(a.velocities(), vb)

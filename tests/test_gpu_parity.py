@@ -520,6 +520,53 @@ def test_set_get_state(md):
     assert np.array_equal(xt.cpu().numpy(), b.positions())
 
 
+@pytest.mark.parametrize("case", ["cfg3a_small", "cfg4_small", "alloy_tbsma_boxes", "cfg0"])
+def test_step_get_state_equals_step_then_get_state(md, case, monkeypatch):
+    """md_step_get_state(n, dt, x, v): the download of the positions runs beside the two passes of the last step; the state it
+    returns and the trajectory it leaves are those of md_step(n) + md_get_state, bit for bit (pinned and pageable host
+    buffers, across rebuilds, echoed back through md_set_state as bench.py's end-to-end leg does; device buffers, the
+    predictor-corrector integrator and a barostat take the plain path)."""
+    import torch
+    monkeypatch.setenv("MD_FORK_MIN_ATOMS", "0")                              # these systems are below the size from which the call forks
+    w = CASES[case]()
+    a, b = md.MDSystem(w), md.MDSystem(w)
+    n = w.n_atoms
+    px, pv = torch.empty((n, 3), dtype=torch.float64).pin_memory().numpy(), torch.empty((n, 3), dtype=torch.float64).pin_memory().numpy()
+    rebuilds = 0
+    for it, k in enumerate([1, 1, 5, 1, 9, 1, 1, 16, 1, 3]):
+        a.step(k, w.dt)
+        xa, va = a.get_state()
+        if it % 3 == 2:
+            xb, vb = b.step_get_state(k, w.dt)                            # pageable numpy buffers
+        else:
+            xb, vb = b.step_get_state(k, w.dt, out=(px, pv))               # pinned
+        assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+        if it % 2:
+            b.set_state(xb, vb)                                            # echo: the forces stay valid
+        rebuilds = b.stats()["rebuilds"]
+    assert rebuilds >= 2 and a.stats()["rebuilds"] == rebuilds and b.stats()["error_flags"] == 0
+    assert np.array_equal(a.positions(), b.positions()) and np.array_equal(a.velocities(), b.velocities())
+    assert np.array_equal(a.compute_forces()[0], b.compute_forces()[0])
+    # positions only / velocities only / device tensors
+    a.step(2, w.dt)
+    xb, _ = b.step_get_state(2, w.dt, out=(px, None))
+    assert np.array_equal(a.positions(), xb)
+    a.step(1, w.dt)
+    _, vb = b.step_get_state(1, w.dt, out=(None, pv))
+    assert np.array_equal(a.velocities(), vb)
+    a.step(2, w.dt)
+    xt, vt = b.step_get_state(2, w.dt, device_out=True)
+    assert np.array_equal(a.positions(), xt.cpu().numpy()) and np.array_equal(a.velocities(), vt.cpu().numpy())
+    with pytest.raises(md.MDError):
+        b.step_get_state(0, w.dt)
+    # the predictor-corrector integrator: plain path, same answers as step + get_state
+    c, d = md.MDSystem(w), md.MDSystem(w)
+    c.set_integrator(md.MD_INT_GEAR5); d.set_integrator(md.MD_INT_GEAR5)
+    c.step(3, w.dt)
+    xd, vd = d.step_get_state(3, w.dt, out=(px, pv))
+    assert np.array_equal(c.positions(), xd) and np.array_equal(c.velocities(), vd)
+
+
 @pytest.mark.parametrize("case,nsteps", [("cfg0", 100), ("cfg0_perm", 60), ("cfg1_small", 60), ("cfg2_small", 60), ("cfg3b_small", 40),
                                          ("cfg4_small", 60), ("alloy_tbsma_boxes", 60), ("alloy4_tables_rcut", 60)])
 def test_gear_predictor_corrector_trajectory(md, case, nsteps):
